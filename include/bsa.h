@@ -1,0 +1,132 @@
+/*
+ * bsa.h -- C ABI of libbsa: uncertainty-gated block-sparse prefill attention for NVIDIA B200 (sm_100a).
+ *
+ * The calls follow the problem statement of arxiv/paper_2607_07724 (citations: PAPER.md line + eq.):
+ *   bsa_build_block_meta : per-KV-block key pooling          (Eq.1/Eq.6 L74,L293; Eq.2)
+ *   bsa_select           : per-(Q-tile, head) block scoring, causal top-k with forced sink/self,
+ *                          normalised cutoff margin sigma, head mean, per-layer q-quantile trigger,
+ *                          shape-uniform padded kv_idx       (Eq.3-5; A.2-A.9 L296-340)
+ *   bsa_sparse_attn_fwd  : exact online-softmax attention over the selected K/V blocks
+ *                                                            (L43-47, L131, A.10 L342)
+ *   bsa_dense_attn_fwd   : dense causal attention, the "x dense" denominator (L45, L156)
+ *
+ * Conventions
+ *   - Every pointer named Q/K/V/O/meta/kv_idx/kv_count/sigma/sigma_bar/trigger/tau/lse/workspace is a
+ *     DEVICE pointer owned by the caller; the library allocates no device memory and keeps no state
+ *     between calls.  `shape` is a HOST pointer.  `stream` is a cudaStream_t passed as void*.
+ *   - Every call only enqueues work on `stream`; it never synchronises and never touches the
+ *     default stream.
+ *   - Argument checks run on the host before any launch; on a non-zero status nothing was enqueued.
+ *     bsa_last_error() returns a thread-local description of the last failure.
+ *   - Tensors are bf16 with the head dimension contiguous; strides are in elements.  Q and O share
+ *     strides; K and V share strides.  Pointers and row strides must be 16-byte aligned.
+ *   - BLOCK_M == BLOCK_N == shape.block (reading G10).  N_B = Q_t = seqlen / block.
+ *   - GQA (reading G7): query head h uses KV head h / (n_q_heads / n_kv_heads).
+ *   - Inputs are assumed finite.
+ */
+#ifndef BSA_H_
+#define BSA_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  BSA_OK = 0,
+  BSA_ERR_INVALID_ARG = 1,        /* NULL pointer, seqlen % block, heads % kv heads, k_budget < 3,
+                                     q_frac outside [0,1], misaligned pointer or stride */
+  BSA_ERR_UNSUPPORTED = 2,        /* block not in {64,128}, head_dim not in {64,128,256}, not sm_100 */
+  BSA_ERR_WORKSPACE_TOO_SMALL = 3,
+  BSA_ERR_CUDA = 4                /* a CUDA runtime / driver call failed (see bsa_last_error) */
+} bsa_status;
+
+typedef enum {
+  BSA_POLICY_TOPK = 0,            /* K-mean backbone (Eq.1), no expansion      (L157) */
+  BSA_POLICY_ROUTER = 1,          /* K-mean backbone, sigma router              (L159) */
+  BSA_POLICY_QUEST = 2,           /* K-min/K-max backbone (Eq.2), no expansion  (L158) */
+  BSA_POLICY_ROUTER_QUEST = 3     /* K-min/K-max backbone, sigma router         (L160) */
+} bsa_policy;
+
+enum { BSA_META_MEAN = 1, BSA_META_MINMAX = 2 }; /* bit mask for `kinds` */
+#define BSA_RHO 2                                 /* expansion factor rho (L129) */
+
+typedef struct {
+  int32_t batch, seqlen, n_q_heads, n_kv_heads, head_dim, block;
+  int64_t q_stride_b, q_stride_h, q_stride_n;     /* Q and O, in elements */
+  int64_t kv_stride_b, kv_stride_h, kv_stride_n;  /* K and V, in elements */
+} bsa_shape;
+
+/*
+ * Block metadata buffer ("meta"), documented so tests can read it:
+ *   offset 0                      : kmean fp32 [B, Hkv, N_B, d]   (Eq.1: (1/BLOCK_N) sum_j k_j)
+ *   offset bsa_block_meta_offset(shape, BSA_META_MINMAX)
+ *                                 : kmin  bf16 [B, Hkv, N_B, d]   (Eq.2: element-wise min)
+ *   directly after kmin           : kmax  bf16 [B, Hkv, N_B, d]   (Eq.2: element-wise max)
+ * The three planes have fixed offsets regardless of `kinds`; planes not requested are left untouched.
+ * bsa_block_meta_bytes returns the size to allocate (0 on invalid shape).
+ */
+size_t bsa_block_meta_bytes(const bsa_shape* shape, int kinds);
+size_t bsa_block_meta_offset(const bsa_shape* shape, int kind /* BSA_META_MEAN | BSA_META_MINMAX */);
+
+/* Pools K once (one pass, 128-bit loads) into `meta`.  kinds: BSA_META_MEAN | BSA_META_MINMAX. */
+bsa_status bsa_build_block_meta(const bsa_shape* shape, const void* K, int kinds, void* meta,
+                                void* stream);
+
+/* Width W of a kv_idx row: k_budget (TOPK, QUEST) or BSA_RHO * k_budget (router policies). */
+int32_t bsa_kv_width(bsa_policy policy, int32_t k_budget);
+
+size_t bsa_select_workspace_bytes(const bsa_shape* shape, bsa_policy policy, int32_t k_budget);
+
+/*
+ * Selection.  For every Q-tile t (rows [t*block, (t+1)*block)) and query head h:
+ *   tile_score[b] = max_{r in tile} s[r,h,b] for visible blocks b <= t            (Eq.3, reading G4)
+ *     s = (q . kmean_b) / sqrt(d)  (TOPK, ROUTER)   |   s = sum_c max(q_c kmax_c, q_c kmin_c) (QUEST*)
+ *   blocks 0 and t are forced on top (Eq.9); the rest sorted by score descending, ties -> lower
+ *   block index first (reading G6).
+ *   sigma[t,h] (Eq.4 / Eq.11, readings G1, G5):
+ *       t+1 <= k_budget : 1
+ *       else (s~[k-1] - s~[k]) / (s~[f] - s~[k]), f = number of forced blocks; 0 when the
+ *       denominator is 0 (L324)
+ *   sigma_bar[t] = mean_h sigma[t,h] (Eq.12, fp32 sum in ascending h, then / H)
+ *   router policies: m = ceil(q_frac*Q_t - 1e-9); tau = m-th smallest sigma_bar (order statistic,
+ *       readings G3, G15); trigger[t] = sigma_bar[t] <= tau; m == 0 -> no trigger, tau = -1.
+ *       other policies: trigger = 0, tau = -1; q_frac is ignored.
+ *   kv_count[t,h] = min(trigger ? 2k : k, t+1); kv_idx[t,h,0..count) = sorted prefix,
+ *       remaining slots = N_B (sentinel)                                          (Eq.14)
+ * Outputs: kv_idx [B,Hq,Q_t,W] int32, kv_count [B,Hq,Q_t] int32, sigma [B,Hq,Q_t] fp32 (required);
+ *          sigma_bar [B,Q_t] fp32, trigger [B,Q_t] u8, tau [B] fp32 (each may be NULL).
+ * `meta` must hold the planes the policy needs (MEAN for TOPK/ROUTER, MINMAX for QUEST policies).
+ */
+bsa_status bsa_select(const bsa_shape* shape, const void* Q, const void* meta, bsa_policy policy,
+                      int32_t k_budget, double q_frac, int32_t* kv_idx, int32_t* kv_count,
+                      float* sigma, float* sigma_bar, uint8_t* trigger, float* tau, void* workspace,
+                      size_t workspace_bytes, void* stream);
+
+/*
+ * Sparse attention.  For tile t, head h, row i: softmax over keys j <= i of the blocks listed in
+ * kv_idx[b,h,t,0..kv_count) (kv_count may be NULL: all W slots are read), scale <= 0 means
+ * 1/sqrt(head_dim).  Entries >= N_B (sentinel) or > t are skipped; the block equal to t gets the
+ * causal diagonal mask; the order of entries is free; entries of one row must be distinct.
+ * O [B,Hq,N,d] bf16 (Q strides); lse [B,Hq,N] fp32 natural-log-sum-exp of the scaled logits, or NULL.
+ */
+bsa_status bsa_sparse_attn_fwd(const bsa_shape* shape, const void* Q, const void* K, const void* V,
+                               const int32_t* kv_idx, const int32_t* kv_count, int32_t kv_width,
+                               float softmax_scale, void* O, float* lse, void* stream);
+
+/* Dense causal attention with the same kernel design (every visible block). */
+bsa_status bsa_dense_attn_fwd(const bsa_shape* shape, const void* Q, const void* K, const void* V,
+                              float softmax_scale, void* O, float* lse, void* stream);
+
+/* Thread-local, static storage; never NULL. */
+const char* bsa_last_error(void);
+
+/* Library version string, e.g. "bsa 0.1 sm_100a". */
+const char* bsa_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BSA_H_ */
