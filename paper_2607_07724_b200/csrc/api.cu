@@ -1,0 +1,208 @@
+// api.cu -- the C ABI of libbsa (include/bsa.h): argument validation, meta / workspace layout,
+// dispatch to the kernels.  Nothing here touches the device except kernel launches on the caller's
+// stream; no device memory is allocated and no state is kept between calls.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+
+#include "bsa_internal.h"
+
+namespace bsa {
+
+static thread_local char g_err[512] = "";
+
+bsa_status fail(bsa_status code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+bsa_status check_launch(const char* what) {
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(BSA_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+  return BSA_OK;
+}
+
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+MetaLayout meta_layout(const Dims& D) {
+  MetaLayout L;
+  L.elems = static_cast<size_t>(D.B) * D.Hkv * D.NB * D.d;
+  L.off_mean = 0;
+  L.off_min = align_up(L.elems * 4, 256);
+  L.off_max = L.off_min + L.elems * 2;
+  L.off_split = align_up(L.off_max + L.elems * 2, 256);
+  L.bytes = L.off_split + 3 * L.elems * 2;
+  return L;
+}
+
+static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+// Shape checks shared by every entry point.
+static bsa_status make_dims(const bsa_shape* s, Dims* out) {
+  if (!s) return fail(BSA_ERR_INVALID_ARG, "shape is NULL");
+  if (s->batch < 1 || s->seqlen < 1 || s->n_q_heads < 1 || s->n_kv_heads < 1)
+    return fail(BSA_ERR_INVALID_ARG, "batch, seqlen and head counts must be positive");
+  if (s->block != 64 && s->block != 128)
+    return fail(BSA_ERR_UNSUPPORTED, "block %d not in {64, 128}", s->block);
+  if (s->head_dim != 64 && s->head_dim != 128 && s->head_dim != 256)
+    return fail(BSA_ERR_UNSUPPORTED, "head_dim %d not in {64, 128, 256}", s->head_dim);
+  if (s->seqlen % s->block != 0)
+    return fail(BSA_ERR_INVALID_ARG, "seqlen %d is not a multiple of block %d", s->seqlen, s->block);
+  if (s->n_q_heads % s->n_kv_heads != 0)
+    return fail(BSA_ERR_INVALID_ARG, "n_q_heads %d is not a multiple of n_kv_heads %d", s->n_q_heads,
+                s->n_kv_heads);
+  if (s->seqlen / s->block > 65535)
+    return fail(BSA_ERR_UNSUPPORTED, "more than 65535 blocks per sequence");
+  const int64_t st[6] = {s->q_stride_b, s->q_stride_h, s->q_stride_n,
+                         s->kv_stride_b, s->kv_stride_h, s->kv_stride_n};
+  for (int i = 0; i < 6; ++i)
+    if (st[i] < 0 || st[i] % 8 != 0)
+      return fail(BSA_ERR_INVALID_ARG, "strides must be non-negative multiples of 8 elements (16 B)");
+  if (s->q_stride_n < s->head_dim || s->kv_stride_n < s->head_dim)
+    return fail(BSA_ERR_INVALID_ARG, "row stride smaller than head_dim");
+  Dims D;
+  D.B = s->batch; D.N = s->seqlen; D.H = s->n_q_heads; D.Hkv = s->n_kv_heads; D.d = s->head_dim;
+  D.Bn = s->block; D.NB = s->seqlen / s->block; D.G = s->n_q_heads / s->n_kv_heads;
+  D.qsb = s->q_stride_b; D.qsh = s->q_stride_h; D.qsn = s->q_stride_n;
+  D.ksb = s->kv_stride_b; D.ksh = s->kv_stride_h; D.ksn = s->kv_stride_n;
+  *out = D;
+  return BSA_OK;
+}
+
+static bsa_status check_device() {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return fail(BSA_ERR_CUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
+  int major = 0;
+  e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+  if (e != cudaSuccess) return fail(BSA_ERR_CUDA, "cudaDeviceGetAttribute: %s", cudaGetErrorString(e));
+  if (major != 10) return fail(BSA_ERR_UNSUPPORTED, "device is sm_%d0, libbsa needs sm_100", major);
+  return BSA_OK;
+}
+
+static bool policy_ok(int p) { return p >= BSA_POLICY_TOPK && p <= BSA_POLICY_ROUTER_QUEST; }
+static bool is_router(int p) { return p == BSA_POLICY_ROUTER || p == BSA_POLICY_ROUTER_QUEST; }
+
+}  // namespace bsa
+
+using namespace bsa;
+
+extern "C" {
+
+const char* bsa_last_error(void) { return g_err; }
+const char* bsa_version(void) { return "bsa 0.1 sm_100a"; }
+
+size_t bsa_block_meta_bytes(const bsa_shape* shape, int kinds) {
+  Dims D;
+  if (make_dims(shape, &D) != BSA_OK) return 0;
+  if ((kinds & ~(BSA_META_MEAN | BSA_META_MINMAX)) != 0 || kinds == 0) return 0;
+  return meta_layout(D).bytes;
+}
+
+size_t bsa_block_meta_offset(const bsa_shape* shape, int kind) {
+  Dims D;
+  if (make_dims(shape, &D) != BSA_OK) return 0;
+  const MetaLayout L = meta_layout(D);
+  return kind == BSA_META_MINMAX ? L.off_min : L.off_mean;
+}
+
+bsa_status bsa_build_block_meta(const bsa_shape* shape, const void* K, int kinds, void* meta,
+                                void* stream) {
+  Dims D;
+  bsa_status st = make_dims(shape, &D);
+  if (st != BSA_OK) return st;
+  if (!K || !meta) return fail(BSA_ERR_INVALID_ARG, "K or meta is NULL");
+  if ((kinds & ~(BSA_META_MEAN | BSA_META_MINMAX)) != 0 || kinds == 0)
+    return fail(BSA_ERR_INVALID_ARG, "kinds must be a non-empty mask of BSA_META_MEAN | BSA_META_MINMAX");
+  if (!aligned16(K) || (reinterpret_cast<uintptr_t>(meta) & 255u))
+    return fail(BSA_ERR_INVALID_ARG, "K must be 16-byte and meta 256-byte aligned");
+  st = check_device();
+  if (st != BSA_OK) return st;
+  return launch_pool(D, K, kinds, meta, static_cast<cudaStream_t>(stream));
+}
+
+int32_t bsa_kv_width(bsa_policy policy, int32_t k_budget) {
+  if (!policy_ok(policy) || k_budget < 1) return 0;
+  return is_router(policy) ? BSA_RHO * k_budget : k_budget;
+}
+
+size_t bsa_select_workspace_bytes(const bsa_shape* shape, bsa_policy policy, int32_t k_budget) {
+  Dims D;
+  if (make_dims(shape, &D) != BSA_OK || !policy_ok(policy) || k_budget < 3) return 0;
+  const size_t bt = static_cast<size_t>(D.B) * D.NB;
+  return align_up(bt * 4, 256) + align_up(bt, 256) + 256;
+}
+
+bsa_status bsa_select(const bsa_shape* shape, const void* Q, const void* meta, bsa_policy policy,
+                      int32_t k_budget, double q_frac, int32_t* kv_idx, int32_t* kv_count,
+                      float* sigma, float* sigma_bar, uint8_t* trigger, float* tau, void* workspace,
+                      size_t workspace_bytes, void* stream) {
+  Dims D;
+  bsa_status st = make_dims(shape, &D);
+  if (st != BSA_OK) return st;
+  if (!Q || !meta || !kv_idx || !kv_count || !sigma)
+    return fail(BSA_ERR_INVALID_ARG, "Q, meta, kv_idx, kv_count and sigma must not be NULL");
+  if (!policy_ok(policy)) return fail(BSA_ERR_INVALID_ARG, "unknown policy %d", static_cast<int>(policy));
+  if (k_budget < 3) return fail(BSA_ERR_INVALID_ARG, "k_budget %d < 3", k_budget);
+  if (k_budget > 128) return fail(BSA_ERR_UNSUPPORTED, "k_budget %d > 128", k_budget);
+  if (is_router(policy) && !(q_frac >= 0.0 && q_frac <= 1.0))
+    return fail(BSA_ERR_INVALID_ARG, "q_frac %g outside [0, 1]", q_frac);
+  if (!aligned16(Q) || (reinterpret_cast<uintptr_t>(meta) & 255u))
+    return fail(BSA_ERR_INVALID_ARG, "Q must be 16-byte and meta 256-byte aligned");
+  if (D.NB > 8192) return fail(BSA_ERR_UNSUPPORTED, "more than 8192 blocks per sequence in select");
+  const size_t need = bsa_select_workspace_bytes(shape, policy, k_budget);
+  if ((!sigma_bar || !trigger) && (!workspace || workspace_bytes < need))
+    return fail(BSA_ERR_WORKSPACE_TOO_SMALL, "workspace of %zu bytes needed, %zu given", need,
+                workspace_bytes);
+  st = check_device();
+  if (st != BSA_OK) return st;
+  const size_t bt = static_cast<size_t>(D.B) * D.NB;
+  char* ws = static_cast<char*>(workspace);
+  if (ws) ws = reinterpret_cast<char*>(align_up(reinterpret_cast<uintptr_t>(ws), 256));
+  if (!sigma_bar) sigma_bar = reinterpret_cast<float*>(ws);
+  if (!trigger) trigger = reinterpret_cast<uint8_t*>(ws + align_up(bt * 4, 256));
+  long long m = 0;  // O9: m = ceil(q*T - 1e-9), clamped to [0, T]
+  if (is_router(policy)) {
+    m = static_cast<long long>(ceil(q_frac * static_cast<double>(D.NB) - 1e-9));
+    if (m < 0) m = 0;
+    if (m > D.NB) m = D.NB;
+  }
+  const int W = bsa_kv_width(policy, k_budget);
+  return launch_select(D, Q, meta, policy, k_budget, W, m, kv_idx, kv_count, sigma, sigma_bar, trigger,
+                       tau, static_cast<cudaStream_t>(stream));
+}
+
+static bsa_status attn_common(const bsa_shape* shape, const void* Q, const void* K, const void* V,
+                              const int32_t* kv_idx, const int32_t* kv_count, int32_t kv_width,
+                              bool sparse, float softmax_scale, void* O, float* lse, void* stream) {
+  Dims D;
+  bsa_status st = make_dims(shape, &D);
+  if (st != BSA_OK) return st;
+  if (!Q || !K || !V || !O) return fail(BSA_ERR_INVALID_ARG, "Q, K, V and O must not be NULL");
+  if (sparse && (!kv_idx || kv_width < 1))
+    return fail(BSA_ERR_INVALID_ARG, "kv_idx is NULL or kv_width < 1");
+  if (!aligned16(Q) || !aligned16(K) || !aligned16(V) || !aligned16(O))
+    return fail(BSA_ERR_INVALID_ARG, "Q, K, V and O must be 16-byte aligned");
+  st = check_device();
+  if (st != BSA_OK) return st;
+  const float scale = softmax_scale > 0.f ? softmax_scale
+                                          : static_cast<float>(1.0 / sqrt(static_cast<double>(D.d)));
+  return launch_attn(D, Q, K, V, kv_idx, kv_count, kv_width, sparse, scale, O, lse,
+                     static_cast<cudaStream_t>(stream));
+}
+
+bsa_status bsa_sparse_attn_fwd(const bsa_shape* shape, const void* Q, const void* K, const void* V,
+                               const int32_t* kv_idx, const int32_t* kv_count, int32_t kv_width,
+                               float softmax_scale, void* O, float* lse, void* stream) {
+  return attn_common(shape, Q, K, V, kv_idx, kv_count, kv_width, true, softmax_scale, O, lse, stream);
+}
+
+bsa_status bsa_dense_attn_fwd(const bsa_shape* shape, const void* Q, const void* K, const void* V,
+                              float softmax_scale, void* O, float* lse, void* stream) {
+  return attn_common(shape, Q, K, V, nullptr, nullptr, 0, false, softmax_scale, O, lse, stream);
+}
+
+}  // extern "C"

@@ -1,0 +1,412 @@
+// attn.cu -- bsa_sparse_attn_fwd / bsa_dense_attn_fwd: exact online-softmax attention over the K/V
+// blocks listed in kv_idx (PAPER.md L43-47 softmax definition; L131, A.10 L342 iteration over
+// kv_idx with a single-compare sentinel skip), and the dense causal kernel of the same design
+// (L45, L156) used as the "x dense" denominator.
+//
+// One CTA per (Q tile, head, batch); 6 warps:
+//   warps 0-3  softmax: tcgen05.ld of S, fp32 online softmax in base 2, P (bf16) -> shared memory,
+//              lazy rescale of the O accumulator in TMEM, final normalisation and store
+//   warp 4     TMA producer: Q once, then K and V 64-key sub-blocks through a ring of stages; the
+//              row coordinate of each load is kv_idx * block ("gather" = ordinary tiled TMA loads)
+//   warp 5     one thread issues tcgen05.mma: S = Q K^T (both K-major, 128B swizzle) into TMEM and
+//              O += P V (V is the MN-major B operand) into TMEM
+// Q tile rows: sparse = one selection tile (BM = block), dense = 128.  For BM = 64 the accumulator
+// rows live in lanes 0-15 of each TMEM sub-partition (UMMA M = 64 layout).
+#include <cuda_bf16.h>
+
+#include "bsa_internal.h"
+#include "sm100_ptx.cuh"
+
+namespace bsa {
+
+namespace {
+
+constexpr int BN = 64;                 // keys per pipeline stage / per S tile
+constexpr int kSoftmaxThreads = 128;
+constexpr int kThreads = 192;
+constexpr int kMaxW = 256;             // widest kv_idx row staged in shared memory
+
+template <int BM, int D>
+struct Cfg {
+  static constexpr int kOcc = (D <= 128) ? 2 : 1;  // CTAs per SM this kernel is sized for
+  static constexpr int Q_BYTES = BM * D * 2;
+  static constexpr int P_BYTES = BM * BN * 2;
+  static constexpr int KV_BYTES = BN * D * 2;
+  static constexpr int kBudget = (kOcc == 2 ? 115712 : 231424) - 1024;  // barriers + list live in 1 KB
+  static constexpr int kNSraw = (kBudget - Q_BYTES - P_BYTES) / KV_BYTES;
+  static constexpr int NS = kNSraw > 8 ? 8 : kNSraw;
+  static constexpr int SMEM = Q_BYTES + P_BYTES + NS * KV_BYTES + 1024;
+  static constexpr uint32_t TMEM_COLS = (D == 64) ? 128 : (D == 128 ? 256 : 512);
+  static constexpr int O_COL = 64;  // S occupies columns [0,64), O columns [64, 64+D)
+  static_assert(NS >= 2, "not enough shared memory for a K/V ring");
+};
+
+struct Params {
+  const int32_t* kv_idx;    // [B,H,T,W] or nullptr (dense)
+  const int32_t* kv_count;  // [B,H,T] or nullptr
+  uint16_t* O;
+  float* lse;
+  int W, B, H, G, N, Bn, NB, NT;
+  int64_t qsb, qsh, qsn;
+  float scale_log2;
+};
+
+// bookkeeping block at the end of dynamic shared memory
+struct alignas(8) Ctl {
+  uint64_t q_full, s_full, s_free, p_full, o_done;
+  uint64_t kv_full[8], kv_empty[8];
+  uint32_t tmem_base;
+  int32_t n_valid;
+  uint16_t list[kMaxW];
+};
+static_assert(sizeof(Ctl) <= 1024, "Ctl must fit the 1 KB bookkeeping area");
+
+template <int BM, int D, bool SPARSE>
+__global__ void __launch_bounds__(kThreads, Cfg<BM, D>::kOcc)
+attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
+            const __grid_constant__ CUtensorMap tmV, const Params p) {
+  using C = Cfg<BM, D>;
+  extern __shared__ __align__(1024) uint8_t smem[];
+  uint8_t* q_s = smem;
+  uint8_t* p_s = smem + C::Q_BYTES;
+  uint8_t* kv_s = p_s + C::P_BYTES;
+  Ctl* ctl = reinterpret_cast<Ctl*>(kv_s + C::NS * C::KV_BYTES);
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  // work item: heaviest (largest tile index) first
+  const int per_tile = p.B * p.H;
+  const int tq = p.NT - 1 - static_cast<int>(blockIdx.x) / per_tile;
+  const int rem = static_cast<int>(blockIdx.x) % per_tile;
+  const int b = rem / p.H, h = rem % p.H, g = h / p.G;
+  const int q0 = tq * BM;  // first query row of this tile
+
+  if ((smem_u32(smem) & 1023u) != 0) __trap();
+
+  // ---- setup ---------------------------------------------------------------------------------
+  if (warp == 5 && lane == 0) {
+    mbar_init(smem_u32(&ctl->q_full), 1);
+    mbar_init(smem_u32(&ctl->s_full), 1);
+    mbar_init(smem_u32(&ctl->s_free), 4);
+    mbar_init(smem_u32(&ctl->p_full), 4);
+    mbar_init(smem_u32(&ctl->o_done), 1);
+    for (int s = 0; s < C::NS; ++s) {
+      mbar_init(smem_u32(&ctl->kv_full[s]), 1);
+      mbar_init(smem_u32(&ctl->kv_empty[s]), 1);
+    }
+    fence_mbar_init();
+  }
+  if (warp == 4) {
+    if (lane == 0) {
+      tma_prefetch_desc(&tmQ);
+      tma_prefetch_desc(&tmK);
+      tma_prefetch_desc(&tmV);
+    }
+    __syncwarp();
+    tmem_alloc<C::TMEM_COLS>(smem_u32(&ctl->tmem_base));
+  }
+  if (SPARSE && warp == 0) {
+    // compact the valid entries of this kv_idx row (sentinel >= N_B and blocks > t are skipped, A.10)
+    const int64_t row = (static_cast<int64_t>(b) * p.H + h) * p.NT + tq;
+    int cnt = p.kv_count ? p.kv_count[row] : p.W;
+    cnt = cnt < 0 ? 0 : (cnt > p.W ? p.W : cnt);
+    const int32_t* src = p.kv_idx + row * p.W;
+    int base = 0;
+    for (int i0 = 0; i0 < cnt; i0 += 32) {
+      const int i = i0 + lane;
+      const int blk = (i < cnt) ? src[i] : -1;
+      const bool ok = (blk >= 0) && (blk < p.NB) && (blk <= tq);
+      const unsigned bal = __ballot_sync(0xffffffffu, ok);
+      if (ok) ctl->list[base + __popc(bal & ((1u << lane) - 1u))] = static_cast<uint16_t>(blk);
+      base += __popc(bal);
+    }
+    if (lane == 0) ctl->n_valid = base;
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = ctl->tmem_base;
+
+  constexpr int SUBS = SPARSE ? (BM / BN) : 1;  // 64-key sub-blocks per selected block
+  int n_it;
+  if (SPARSE) {
+    n_it = ctl->n_valid * SUBS;
+  } else {
+    const int last = (q0 + BM < p.N ? q0 + BM : p.N);
+    n_it = last / BN;
+  }
+  auto key_start = [&](int j) -> int {
+    if (SPARSE) return ctl->list[j / SUBS] * p.Bn + (j % SUBS) * BN;
+    return j * BN;
+  };
+
+  if (n_it > 0) {
+    if (warp == 4) {
+      // ---- TMA producer ----------------------------------------------------------------------
+      if (lane == 0) {
+        mbar_arrive_expect_tx(smem_u32(&ctl->q_full), C::Q_BYTES);
+        tma_load_5d(smem_u32(q_s), &tmQ, smem_u32(&ctl->q_full), 0, q0, 0, h, b);
+        for (int j = 0; j < n_it; ++j) {
+          const int k0 = key_start(j);
+#pragma unroll
+          for (int kv = 0; kv < 2; ++kv) {
+            const int it = 2 * j + kv, s = it % C::NS;
+            mbar_wait(smem_u32(&ctl->kv_empty[s]), ((it / C::NS) & 1) ^ 1);
+            mbar_arrive_expect_tx(smem_u32(&ctl->kv_full[s]), C::KV_BYTES);
+            tma_load_5d(smem_u32(kv_s + s * C::KV_BYTES), kv ? &tmV : &tmK,
+                        smem_u32(&ctl->kv_full[s]), 0, k0, 0, g, b);
+          }
+        }
+      }
+    } else if (warp == 5) {
+      // ---- MMA issuer ------------------------------------------------------------------------
+      if (lane == 0) {
+        constexpr uint32_t idesc_qk = umma_idesc_bf16(BM, BN, 0, 0);
+        constexpr uint32_t idesc_pv = umma_idesc_bf16(BM, D, 0, 1);
+        const uint32_t tS = tmem, tO = tmem + C::O_COL;
+        const uint32_t q_a = smem_u32(q_s), p_a = smem_u32(p_s), kv_a = smem_u32(kv_s);
+        mbar_wait(smem_u32(&ctl->q_full), 0);
+        for (int j = 0; j <= n_it; ++j) {
+          if (j < n_it) {  // S(j) = Q K_j^T
+            const int it = 2 * j, s = it % C::NS;
+            mbar_wait(smem_u32(&ctl->kv_full[s]), (it / C::NS) & 1);
+            if (j > 0) mbar_wait(smem_u32(&ctl->s_free), (j - 1) & 1);
+            tc_fence_after();
+            const uint32_t k_a = kv_a + s * C::KV_BYTES;
+#pragma unroll
+            for (int ks = 0; ks < D / 16; ++ks) {
+              const uint64_t ad = umma_smem_desc(q_a + (ks >> 2) * (BM * 128) + (ks & 3) * 32, 16, 1024);
+              const uint64_t bd = umma_smem_desc(k_a + (ks >> 2) * (BN * 128) + (ks & 3) * 32, 16, 1024);
+              umma_ss(tS, ad, bd, idesc_qk, ks > 0);
+            }
+            tc_commit(smem_u32(&ctl->kv_empty[s]));
+            tc_commit(smem_u32(&ctl->s_full));
+          }
+          if (j > 0) {  // O += P(j-1) V_{j-1}
+            const int jj = j - 1, it = 2 * jj + 1, s = it % C::NS;
+            mbar_wait(smem_u32(&ctl->kv_full[s]), (it / C::NS) & 1);
+            mbar_wait(smem_u32(&ctl->p_full), jj & 1);
+            tc_fence_after();
+            const uint32_t v_a = kv_a + s * C::KV_BYTES;
+#pragma unroll
+            for (int ks = 0; ks < BN / 16; ++ks) {
+              const uint64_t ad = umma_smem_desc(p_a + ks * 32, 16, 1024);
+              const uint64_t bd = umma_smem_desc(v_a + ks * 2048, BN * 128, 1024);
+              umma_ss(tO, ad, bd, idesc_pv, (jj > 0) || (ks > 0));
+            }
+            tc_commit(smem_u32(&ctl->kv_empty[s]));
+            tc_commit(smem_u32(&ctl->o_done));
+          }
+        }
+      }
+    } else {
+      // ---- softmax warps ---------------------------------------------------------------------
+      const bool active = (BM == 128) || (lane < 16);
+      const int r = (BM == 128) ? tid : (warp * 16 + (lane & 15));
+      const int qrow = q0 + r;
+      const uint32_t lane_base = static_cast<uint32_t>(warp * 32) << 16;
+      const uint32_t tS = tmem + lane_base, tO = tmem + lane_base + C::O_COL;
+      float m = -INFINITY, l = 0.f;
+      for (int j = 0; j < n_it; ++j) {
+        const int k0 = key_start(j);
+        mbar_wait(smem_u32(&ctl->s_full), j & 1);
+        tc_fence_after();
+        uint32_t sa[32], sb[32];
+        tmem_ld32(tS, sa);
+        tmem_ld32(tS + 32, sb);
+        tmem_ld_wait();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&ctl->s_free));
+
+        float x[64];
+        const bool need_mask = (k0 + BN - 1 > q0);
+#pragma unroll
+        for (int c = 0; c < 32; ++c) {
+          x[c] = __uint_as_float(sa[c]) * p.scale_log2;
+          x[c + 32] = __uint_as_float(sb[c]) * p.scale_log2;
+        }
+        if (need_mask) {
+#pragma unroll
+          for (int c = 0; c < 64; ++c) x[c] = (k0 + c <= qrow) ? x[c] : -INFINITY;
+        }
+        float mx = x[0];
+#pragma unroll
+        for (int c = 1; c < 64; ++c) mx = fmaxf(mx, x[c]);
+        float m_new = fmaxf(m, mx);
+        // lazy rescale: keep the stale reference max unless some row of this warp grew by > 2^8
+        const bool grow = active && (m_new - m > 8.0f);
+        const bool any = __any_sync(0xffffffffu, grow);
+        if (!any) m_new = m;
+        const float alpha = ex2_approx(m - m_new);
+        float sum = 0.f;
+        uint32_t pk[32];
+#pragma unroll
+        for (int c = 0; c < 64; c += 2) {
+          const float e0 = ex2_approx(x[c] - m_new), e1 = ex2_approx(x[c + 1] - m_new);
+          sum += e0 + e1;
+          pk[c >> 1] = pack_bf16x2(e0, e1);
+        }
+        l = l * alpha + sum;
+        m = m_new;
+
+        if (j > 0) {
+          mbar_wait(smem_u32(&ctl->o_done), (j - 1) & 1);  // PV(j-1) done: P and O are ours
+          tc_fence_after();
+          if (any) {
+#pragma unroll
+            for (int c0 = 0; c0 < D; c0 += 32) {
+              uint32_t o[32];
+              tmem_ld32(tO + c0, o);
+              tmem_ld_wait();
+#pragma unroll
+              for (int c = 0; c < 32; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * alpha);
+              tmem_st32(tO + c0, o);
+            }
+            tmem_st_wait();
+          }
+        }
+        if (active) {
+          uint8_t* prow = p_s + r * 128;
+#pragma unroll
+          for (int c = 0; c < 8; ++c) {
+            uint4 v = make_uint4(pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
+            *reinterpret_cast<uint4*>(prow + ((c ^ (r & 7)) << 4)) = v;
+          }
+        }
+        fence_proxy_async_smem();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&ctl->p_full));
+      }
+      // ---- epilogue: O / l -> bf16 -> global ---------------------------------------------------
+      mbar_wait(smem_u32(&ctl->o_done), (n_it - 1) & 1);
+      tc_fence_after();
+      const float inv_l = 1.0f / l;
+      const bool store = active && (qrow < p.N);
+      uint16_t* orow = p.O + b * p.qsb + h * p.qsh + static_cast<int64_t>(qrow) * p.qsn;
+#pragma unroll
+      for (int c0 = 0; c0 < D; c0 += 32) {
+        uint32_t o[32];
+        tmem_ld32(tO + c0, o);
+        tmem_ld_wait();
+        if (store) {
+#pragma unroll
+          for (int c = 0; c < 32; c += 8) {
+            uint4 v;
+            v.x = pack_bf16x2(__uint_as_float(o[c]) * inv_l, __uint_as_float(o[c + 1]) * inv_l);
+            v.y = pack_bf16x2(__uint_as_float(o[c + 2]) * inv_l, __uint_as_float(o[c + 3]) * inv_l);
+            v.z = pack_bf16x2(__uint_as_float(o[c + 4]) * inv_l, __uint_as_float(o[c + 5]) * inv_l);
+            v.w = pack_bf16x2(__uint_as_float(o[c + 6]) * inv_l, __uint_as_float(o[c + 7]) * inv_l);
+            *reinterpret_cast<uint4*>(orow + c0 + c) = v;
+          }
+        }
+      }
+      if (store && p.lse)
+        p.lse[(static_cast<int64_t>(b) * p.H + h) * p.N + qrow] =
+            (m + log2f(l)) * 0.6931471805599453f;
+      tc_fence_before();
+    }
+  } else if (warp < 4) {
+    // nothing attended (possible only with a caller-provided kv_idx): zeros, lse = -inf
+    const bool active = (BM == 128) || (lane < 16);
+    const int r = (BM == 128) ? tid : (warp * 16 + (lane & 15));
+    const int qrow = q0 + r;
+    if (active && qrow < p.N) {
+      uint16_t* orow = p.O + b * p.qsb + h * p.qsh + static_cast<int64_t>(qrow) * p.qsn;
+      for (int c = 0; c < D; c += 8) *reinterpret_cast<uint4*>(orow + c) = make_uint4(0, 0, 0, 0);
+      if (p.lse) p.lse[(static_cast<int64_t>(b) * p.H + h) * p.N + qrow] = -INFINITY;
+    }
+  }
+
+  // ---- teardown ------------------------------------------------------------------------------
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 4) tmem_dealloc<C::TMEM_COLS>(tmem);
+}
+
+// ---- host side ---------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
+                                  const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+  }
+  return fn;
+}
+
+// bf16 tensor [B, heads, N, d] (strides in elements) viewed as 5-D (64, N, d/64, heads, B) so one
+// TMA instruction lands a [rows x d] tile as d/64 consecutive 128B-swizzled [rows x 64] chunks.
+bool make_tmap(CUtensorMap* m, const void* base, int B, int heads, int N, int d, int64_t sb,
+               int64_t sh, int64_t sn, int rows) {
+  EncodeTiledFn fn = encode_fn();
+  if (!fn) return false;
+  cuuint64_t dims[5] = {64, static_cast<cuuint64_t>(N), static_cast<cuuint64_t>(d / 64),
+                        static_cast<cuuint64_t>(heads), static_cast<cuuint64_t>(B)};
+  cuuint64_t strides[4] = {static_cast<cuuint64_t>(sn) * 2, 128, static_cast<cuuint64_t>(sh) * 2,
+                           static_cast<cuuint64_t>(sb) * 2};
+  if (heads == 1) strides[2] = strides[0] * static_cast<cuuint64_t>(N);
+  if (B == 1) strides[3] = strides[2] * static_cast<cuuint64_t>(heads);
+  cuuint32_t box[5] = {64, static_cast<cuuint32_t>(rows), static_cast<cuuint32_t>(d / 64), 1, 1};
+  cuuint32_t es[5] = {1, 1, 1, 1, 1};
+  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 5, const_cast<void*>(base), dims, strides, box,
+                  es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                  CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS;
+}
+
+template <int BM, int D, bool SPARSE>
+bsa_status run(const Dims& S, const void* Q, const void* K, const void* V, const Params& prm,
+               cudaStream_t stream) {
+  using C = Cfg<BM, D>;
+  CUtensorMap tq, tk, tv;
+  if (!make_tmap(&tq, Q, S.B, S.H, S.N, S.d, S.qsb, S.qsh, S.qsn, BM) ||
+      !make_tmap(&tk, K, S.B, S.Hkv, S.N, S.d, S.ksb, S.ksh, S.ksn, BN) ||
+      !make_tmap(&tv, V, S.B, S.Hkv, S.N, S.d, S.ksb, S.ksh, S.ksn, BN))
+    return fail(BSA_ERR_CUDA, "attn: cuTensorMapEncodeTiled failed");
+  auto kern = attn_kernel<BM, D, SPARSE>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM);
+  if (e != cudaSuccess) return fail(BSA_ERR_CUDA, "attn: smem attribute: %s", cudaGetErrorString(e));
+  const unsigned grid = static_cast<unsigned>(prm.NT) * prm.B * prm.H;
+  kern<<<grid, kThreads, C::SMEM, stream>>>(tq, tk, tv, prm);
+  return check_launch("attn_kernel");
+}
+
+}  // namespace
+
+bsa_status launch_attn(const Dims& S, const void* Q, const void* K, const void* V,
+                       const int32_t* kv_idx, const int32_t* kv_count, int W, bool sparse, float scale,
+                       void* O, float* lse, cudaStream_t stream) {
+  Params prm;
+  prm.kv_idx = kv_idx;
+  prm.kv_count = kv_count;
+  prm.O = static_cast<uint16_t*>(O);
+  prm.lse = lse;
+  prm.W = W;
+  prm.B = S.B; prm.H = S.H; prm.G = S.G; prm.N = S.N; prm.Bn = S.Bn; prm.NB = S.NB;
+  prm.qsb = S.qsb; prm.qsh = S.qsh; prm.qsn = S.qsn;
+  prm.scale_log2 = scale * 1.4426950408889634f;
+  if (sparse) {
+    if (W > kMaxW) return fail(BSA_ERR_UNSUPPORTED, "sparse attn: kv_width %d > %d", W, kMaxW);
+    prm.NT = S.NB;
+#define BSA_SP(BMM, DD) \
+  if (S.Bn == BMM && S.d == DD) return run<BMM, DD, true>(S, Q, K, V, prm, stream);
+    BSA_SP(64, 64) BSA_SP(64, 128) BSA_SP(64, 256) BSA_SP(128, 64) BSA_SP(128, 128) BSA_SP(128, 256)
+#undef BSA_SP
+  } else {
+    prm.NT = (S.N + 127) / 128;
+    if (S.d == 64) return run<128, 64, false>(S, Q, K, V, prm, stream);
+    if (S.d == 128) return run<128, 128, false>(S, Q, K, V, prm, stream);
+    if (S.d == 256) return run<128, 256, false>(S, Q, K, V, prm, stream);
+  }
+  return fail(BSA_ERR_UNSUPPORTED, "attn: unsupported head_dim %d / block %d", S.d, S.Bn);
+}
+
+}  // namespace bsa

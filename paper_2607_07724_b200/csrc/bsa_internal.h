@@ -1,0 +1,43 @@
+// bsa_internal.h -- host-side declarations shared by the translation units of libbsa.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "../../include/bsa.h"
+
+namespace bsa {
+
+// Validated problem dimensions (derived from bsa_shape).
+struct Dims {
+  int B, N, H, Hkv, d, Bn, NB, G;
+  int64_t qsb, qsh, qsn;  // Q / O strides in elements
+  int64_t ksb, ksh, ksn;  // K / V strides in elements
+};
+
+bsa_status fail(bsa_status code, const char* fmt, ...);
+bsa_status check_launch(const char* what);
+
+// meta plane offsets in bytes (see include/bsa.h); the three bf16 split planes of kmean
+// (hi, mid, lo; hi+mid+lo == kmean exactly) follow kmax and feed the tensor-core scoring.
+struct MetaLayout {
+  size_t elems;      // B*Hkv*NB*d
+  size_t off_mean;   // fp32
+  size_t off_min;    // bf16
+  size_t off_max;    // bf16
+  size_t off_split;  // bf16 x 3 planes
+  size_t bytes;
+};
+MetaLayout meta_layout(const Dims& D);
+
+// kernels (each only enqueues on `stream`)
+bsa_status launch_pool(const Dims& D, const void* K, int kinds, void* meta, cudaStream_t stream);
+bsa_status launch_select(const Dims& D, const void* Q, const void* meta, int policy, int k, int W,
+                         long long m_route, int32_t* kv_idx, int32_t* kv_count, float* sigma,
+                         float* sigma_bar, uint8_t* trigger, float* tau, cudaStream_t stream);
+bsa_status launch_attn(const Dims& D, const void* Q, const void* K, const void* V,
+                       const int32_t* kv_idx, const int32_t* kv_count, int W, bool sparse,
+                       float scale, void* O, float* lse, cudaStream_t stream);
+
+}  // namespace bsa

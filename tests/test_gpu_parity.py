@@ -1,0 +1,308 @@
+"""GPU-vs-oracle parity through the C ABI (pytest -m gpu).  Every stage is compared element by
+element with the CPU oracle on the same seeded inputs: small cases in full, BASELINE.json's full-size
+configuration C2 (the one bench.py times) with the full oracle selection and sampled attention tiles.
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2607_07724_b200 import synth
+
+from parity_util import (bf16_bits, bf16_to_f32, compare_attn, compare_select, to_torch_bf16)
+
+pytestmark = pytest.mark.gpu
+
+OUT_DIR = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+
+
+@pytest.fixture(scope="module")
+def bsa():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2607_07724_b200 import binding
+    binding.load_library()
+    return binding
+
+
+def _small_cases():
+    C = synth.CONFIGS
+    return {
+        "C1": C["C1"],
+        "C2s": C["C2"].scaled(4096, "C2s"),
+        "C4s": C["C4"].scaled(8192, "C4s"),
+        "C5s": C["C5"].scaled(8192, "C5s"),
+        "C1odd": C["C1"].scaled(64 * 5, "C1odd"),     # ragged: odd number of 64-row tiles
+    }
+
+
+_CACHE = {}
+
+
+def _case(name):
+    """inputs + oracle pooling, cached per session"""
+    if name not in _CACHE:
+        cfg = _small_cases().get(name) or synth.CONFIGS[name]
+        inp = synth.make_inputs(cfg)
+        meta = oracle.pool(inp.K, cfg.block)
+        _CACHE[name] = (cfg, inp, meta)
+    return _CACHE[name]
+
+
+def _dev(inp):
+    Q = to_torch_bf16(inp.Q)[None]
+    K = to_torch_bf16(inp.K)[None]
+    V = to_torch_bf16(inp.V)[None]
+    return Q, K, V
+
+
+def _meta_from_oracle(bsa, meta_np, K, block):
+    """Device meta buffer filled with the ORACLE's pooled planes (stage-wise comparison)."""
+    import torch
+    kmean, kmin, kmax = meta_np
+    buf = bsa.bsa_build_block_meta(K, block, 3)          # also fills the internal split planes
+    vm, vn, vx = bsa.meta_views(buf, K.shape, block)
+    vm.copy_(torch.from_numpy(kmean)[None])
+    vn.copy_(to_torch_bf16(kmin)[None])
+    vx.copy_(to_torch_bf16(kmax)[None])
+    return buf
+
+
+def _log(name, payload):
+    os.makedirs(OUT_DIR, exist_ok=True)
+    with open(os.path.join(OUT_DIR, "tie_log.jsonl"), "a") as f:
+        f.write(json.dumps(dict(case=name, **payload)) + "\n")
+
+
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["C1", "C2s", "C4s", "C5s", "C1odd"])
+def test_pool_parity(bsa, name):
+    import torch
+    cfg, inp, meta_np = _case(name)
+    _, K, _ = _dev(inp)
+    buf = bsa.bsa_build_block_meta(K, cfg.block, 3)
+    torch.cuda.synchronize()
+    kmean, kmin, kmax = bsa.meta_views(buf, K.shape, cfg.block)
+    # fp64 block sums are exact, so the mean is the correctly rounded one: bit-exact with the oracle
+    assert np.array_equal(kmean[0].cpu().numpy().view(np.uint32), meta_np[0].view(np.uint32))
+    # min / max equal as numbers (-0 == +0)
+    assert np.array_equal(bf16_to_f32(bf16_bits(kmin[0])), bf16_to_f32(meta_np[1]))
+    assert np.array_equal(bf16_to_f32(bf16_bits(kmax[0])), bf16_to_f32(meta_np[2]))
+
+
+def test_pool_strided_and_batched(bsa):
+    """batch 2, K given as a strided view ([B, N, Hkv, d] storage): same result as contiguous"""
+    import torch
+    cfg, inp, meta_np = _case("C1")
+    K1 = to_torch_bf16(inp.K)
+    Kb = torch.stack([K1, K1.flip(1)])                       # [2, Hkv, N, d]
+    Kst = Kb.permute(0, 2, 1, 3).contiguous().permute(0, 2, 1, 3)   # same values, NHD storage
+    assert not Kst.is_contiguous()
+    a = bsa.bsa_build_block_meta(Kb.contiguous(), cfg.block, 3)
+    b = bsa.bsa_build_block_meta(Kst, cfg.block, 3)
+    torch.cuda.synchronize()
+    assert torch.equal(a, b)
+    kmean, _, _ = bsa.meta_views(a, Kb.shape, cfg.block)
+    assert np.array_equal(kmean[0].cpu().numpy().view(np.uint32), meta_np[0].view(np.uint32))
+
+
+def _gpu_select_np(r):
+    return dict(kv_idx=r["kv_idx"][0].cpu().numpy(), kv_count=r["kv_count"][0].cpu().numpy(),
+                sigma=r["sigma"][0].cpu().numpy(), sigma_bar=r["sigma_bar"][0].cpu().numpy(),
+                trigger=r["trigger"][0].cpu().numpy(), tau=float(r["tau"][0].item()))
+
+
+SELECT_CASES = [("C1", p, 0.25) for p in ("topk", "router", "quest", "router_quest")] + \
+               [("C2s", p, 0.25) for p in ("topk", "router", "quest", "router_quest")] + \
+               [("C4s", "quest", 0.25), ("C4s", "router_quest", 0.1), ("C4s", "router_quest", 0.5),
+                ("C5s", "router", 0.25), ("C5s", "router_quest", 0.25),
+                ("C1odd", "router", 0.25), ("C1", "router", 0.0), ("C1", "router_quest", 1.0)]
+
+
+@pytest.mark.parametrize("name,policy,q", SELECT_CASES)
+def test_select_parity_stagewise(bsa, name, policy, q):
+    """bsa_select fed the ORACLE's pooled keys vs oracle O3-O10: kv_idx / kv_count / trigger bit-exact
+    outside the logged tie bands, sigma within 1e-4."""
+    import torch
+    cfg, inp, meta_np = _case(name)
+    Q, K, _ = _dev(inp)
+    buf = _meta_from_oracle(bsa, meta_np, K, cfg.block)
+    r = bsa.bsa_select(Q, buf, K, cfg.block, policy, cfg.k_budget, q)
+    torch.cuda.synchronize()
+    orc = oracle.select(inp.Q, meta_np, cfg.block, policy, cfg.k_budget, q, want_scores=True)
+    log = []
+    stats = compare_select(_gpu_select_np(r), orc, cfg.n_blocks, cfg.k_budget, log)
+    _log(f"{name}/{policy}/q{q}", dict(stage="select", **stats))
+    assert stats["tie_rows"] <= 0.05 * stats["rows"] + 4
+
+
+@pytest.mark.parametrize("name", ["C1", "C2s", "C5s", "C1odd"])
+def test_dense_attention_parity(bsa, name):
+    import torch
+    cfg, inp, _ = _case(name)
+    Q, K, V = _dev(inp)
+    O, lse = bsa.bsa_dense_attn_fwd(Q, K, V, cfg.block, want_lse=True)
+    torch.cuda.synchronize()
+    T, H = cfg.n_blocks, cfg.n_q_heads
+    if name == "C1" or name == "C1odd":
+        pairs = [(t, h) for h in range(H) for t in range(T)]
+    else:
+        ts = sorted(set([0, 1, 2, T // 2, T - 2, T - 1]))
+        pairs = [(t, h) for h in (0, H // 2, H - 1) for t in ts]
+    ref, ref_lse = oracle.attn_pairs(inp.Q, inp.K, inp.V, cfg.block, pairs)
+    Og = O[0].float().cpu().numpy().reshape(H, T, cfg.block, cfg.head_dim)
+    Lg = lse[0].cpu().numpy().reshape(H, T, cfg.block)
+    got = np.stack([Og[h, t] for t, h in pairs])
+    got_lse = np.stack([Lg[h, t] for t, h in pairs])
+    compare_attn(got, ref, f"dense {name}")
+    np.testing.assert_allclose(got_lse, ref_lse, rtol=0, atol=2e-3)
+
+
+ATTN_CASES = [("C1", "topk"), ("C1", "router"), ("C2s", "router_quest"), ("C2s", "topk"),
+              ("C4s", "router_quest"), ("C5s", "router"), ("C5s", "router_quest"), ("C1odd", "router")]
+
+
+@pytest.mark.parametrize("name,policy", ATTN_CASES)
+def test_sparse_attention_parity_stagewise(bsa, name, policy):
+    """bsa_sparse_attn_fwd fed the ORACLE's kv_idx vs oracle O11."""
+    import torch
+    cfg, inp, meta_np = _case(name)
+    Q, K, V = _dev(inp)
+    orc = oracle.select(inp.Q, meta_np, cfg.block, policy, cfg.k_budget, 0.25)
+    kv_idx = torch.from_numpy(orc["kv_idx"])[None].cuda()
+    kv_count = torch.from_numpy(orc["kv_count"])[None].cuda()
+    O, lse = bsa.bsa_sparse_attn_fwd(Q, K, V, kv_idx, kv_count, cfg.block, want_lse=True)
+    torch.cuda.synchronize()
+    T, H = cfg.n_blocks, cfg.n_q_heads
+    if T * H <= 256:
+        pairs = [(t, h) for h in range(H) for t in range(T)]
+    else:
+        ts = sorted(set([0, 1, 2, 3, cfg.k_budget - 1, cfg.k_budget, min(T - 1, 2 * cfg.k_budget), T // 2,
+                         T - 2, T - 1]))
+        ts = [t for t in ts if 0 <= t < T]
+        pairs = [(t, h) for h in sorted(set([0, 1, H // 2, H - 1])) for t in ts]
+    ref, ref_lse = oracle.attn_pairs(inp.Q, inp.K, inp.V, cfg.block, pairs, orc["kv_idx"], orc["kv_count"])
+    Og = O[0].float().cpu().numpy().reshape(H, T, cfg.block, cfg.head_dim)
+    Lg = lse[0].cpu().numpy().reshape(H, T, cfg.block)
+    got = np.stack([Og[h, t] for t, h in pairs])
+    got_lse = np.stack([Lg[h, t] for t, h in pairs])
+    compare_attn(got, ref, f"sparse {name}/{policy}")
+    np.testing.assert_allclose(got_lse, ref_lse, rtol=0, atol=2e-3)
+
+
+def test_sparse_attention_edge_cases(bsa):
+    """permuted rows, sentinel / future entries skipped, kv_count = NULL, empty rows -> zeros,
+    k_budget >= N_B reduces to dense."""
+    import torch
+    cfg, inp, meta_np = _case("C1")
+    Q, K, V = _dev(inp)
+    T, H, NB = cfg.n_blocks, cfg.n_q_heads, cfg.n_blocks
+    orc = oracle.select(inp.Q, meta_np, cfg.block, "router", cfg.k_budget, 0.25)
+    rng = np.random.default_rng(0)
+    W = orc["kv_idx"].shape[-1]
+    idx = orc["kv_idx"].copy()
+    # sentinel padding stays, add blocks from the future (must be skipped), then permute each row
+    for h in range(H):
+        for t in range(T):
+            row = idx[h, t]
+            free = np.nonzero(row == NB)[0]
+            if len(free) and t + 1 < NB:
+                row[free[0]] = t + 1
+            idx[h, t] = rng.permutation(row)
+    idx[1, 5, :] = NB                                   # nothing attended
+    kv_idx = torch.from_numpy(idx)[None].cuda()
+    O, lse = bsa.bsa_sparse_attn_fwd(Q, K, V, kv_idx, None, cfg.block, want_lse=True)
+    torch.cuda.synchronize()
+    pairs = [(t, h) for h in range(H) for t in range(T)]
+    ref, ref_lse = oracle.attn_pairs(inp.Q, inp.K, inp.V, cfg.block, pairs, idx, None)
+    got = O[0].float().cpu().numpy().reshape(H * T, cfg.block, cfg.head_dim)
+    compare_attn(got, ref, "sparse edge")
+    assert (got.reshape(H, T, -1)[1, 5] == 0).all()
+    assert np.isneginf(lse[0, 1].cpu().numpy().reshape(T, cfg.block)[5]).all()
+    # k_budget >= N_B: every visible block selected -> equals the dense kernel's result
+    full = oracle.select(inp.Q, meta_np, cfg.block, "topk", NB, 0.25)
+    O2, _ = bsa.bsa_sparse_attn_fwd(Q, K, V, torch.from_numpy(full["kv_idx"])[None].cuda(),
+                                    torch.from_numpy(full["kv_count"])[None].cuda(), cfg.block)
+    Od, _ = bsa.bsa_dense_attn_fwd(Q, K, V, cfg.block)
+    torch.cuda.synchronize()
+    refd, _ = oracle.attn_pairs(inp.Q, inp.K, inp.V, cfg.block, pairs)
+    compare_attn(O2[0].float().cpu().numpy().reshape(H * T, cfg.block, -1), refd, "sparse k>=N_B")
+    assert (O2.float() - Od.float()).abs().max().item() <= 2e-2
+
+
+@pytest.mark.parametrize("name,policy", [("C1", "router"), ("C2s", "router_quest"), ("C5s", "router")])
+def test_end_to_end_chain(bsa, name, policy):
+    """pool -> select -> sparse attention chained on the GPU vs the oracle chain."""
+    import torch
+    cfg, inp, meta_np = _case(name)
+    Q, K, V = _dev(inp)
+    buf = bsa.bsa_build_block_meta(K, cfg.block, 3)
+    r = bsa.bsa_select(Q, buf, K, cfg.block, policy, cfg.k_budget, 0.25)
+    O, _ = bsa.bsa_sparse_attn_fwd(Q, K, V, r["kv_idx"], r["kv_count"], cfg.block)
+    torch.cuda.synchronize()
+    orc = oracle.select(inp.Q, meta_np, cfg.block, policy, cfg.k_budget, 0.25, want_scores=True)
+    log = []
+    stats = compare_select(_gpu_select_np(r), orc, cfg.n_blocks, cfg.k_budget, log)
+    tied = {(e[1], e[2]) for e in log if e[0] == "kv_idx"}
+    flipped_t = {e[1] for e in log if e[0] == "trigger"}
+    T, H = cfg.n_blocks, cfg.n_q_heads
+    ts = sorted(set([0, 1, cfg.k_budget, T // 2, T - 1]))
+    pairs = [(t, h) for h in sorted(set([0, H - 1])) for t in ts
+             if (h, t) not in tied and t not in flipped_t]
+    ref, _ = oracle.attn_pairs(inp.Q, inp.K, inp.V, cfg.block, pairs, orc["kv_idx"], orc["kv_count"])
+    Og = O[0].float().cpu().numpy().reshape(H, T, cfg.block, cfg.head_dim)
+    compare_attn(np.stack([Og[h, t] for t, h in pairs]), ref, f"e2e {name}/{policy}")
+    _log(f"{name}/{policy}", dict(stage="e2e", **stats))
+
+
+# ---- BASELINE.json configs[1] at full size, the launch configuration bench.py times --------------
+@pytest.mark.parametrize("policy", ["router_quest", "topk"])
+def test_full_size_c2(bsa, policy):
+    import torch
+    cfg, inp, meta_np = _case("C2")
+    Q, K, V = _dev(inp)
+    buf = bsa.bsa_build_block_meta(K, cfg.block, 3)
+    kmean, kmin, kmax = bsa.meta_views(buf, K.shape, cfg.block)
+    assert np.array_equal(kmean[0].cpu().numpy().view(np.uint32), meta_np[0].view(np.uint32))
+    assert np.array_equal(bf16_to_f32(bf16_bits(kmax[0])), bf16_to_f32(meta_np[2]))
+    r = bsa.bsa_select(Q, buf, K, cfg.block, policy, cfg.k_budget, 0.25)
+    O, _ = bsa.bsa_sparse_attn_fwd(Q, K, V, r["kv_idx"], r["kv_count"], cfg.block)
+    Od, _ = bsa.bsa_dense_attn_fwd(Q, K, V, cfg.block)
+    torch.cuda.synchronize()
+    orc = oracle.select(inp.Q, meta_np, cfg.block, policy, cfg.k_budget, 0.25, want_scores=True)
+    log = []
+    stats = compare_select(_gpu_select_np(r), orc, cfg.n_blocks, cfg.k_budget, log)
+    _log(f"C2/{policy}", dict(stage="full", **stats))
+    tied = {(e[1], e[2]) for e in log if e[0] == "kv_idx"}
+    flipped_t = {e[1] for e in log if e[0] == "trigger"}
+    T, H = cfg.n_blocks, cfg.n_q_heads
+    ts = [0, 1, 31, 32, 63, 64, 65, 200, 383, 511]
+    needle_pairs = [(n["q_row"] // cfg.block, n["head"]) for n in inp.needles[:4]]
+    pairs = [(t, h) for h in (0, 13, 27) for t in ts] + needle_pairs
+    pairs = [(t, h) for t, h in pairs if (h, t) not in tied and t not in flipped_t]
+    ref, _ = oracle.attn_pairs(inp.Q, inp.K, inp.V, cfg.block, pairs, orc["kv_idx"], orc["kv_count"])
+    Og = O[0].float().cpu().numpy().reshape(H, T, cfg.block, cfg.head_dim)
+    compare_attn(np.stack([Og[h, t] for t, h in pairs]), ref, f"C2 sparse {policy}")
+    if policy == "topk":
+        dpairs = [(t, h) for h in (0, 27) for t in (0, 1, 2, 100, 511)]
+        refd, _ = oracle.attn_pairs(inp.Q, inp.K, inp.V, cfg.block, dpairs)
+        Odg = Od[0].float().cpu().numpy().reshape(H, T, cfg.block, cfg.head_dim)
+        compare_attn(np.stack([Odg[h, t] for t, h in dpairs]), refd, "C2 dense")
+    # properties that hold at any size
+    kvc = r["kv_count"][0].cpu().numpy()
+    trig = r["trigger"][0].cpu().numpy().astype(bool)
+    k = cfg.k_budget
+    tt = np.arange(T)
+    expect = np.minimum(np.where(trig, 2 * k, k) if policy.startswith("router") else k, tt + 1)
+    assert (kvc == expect[None, :]).all()
+    if policy.startswith("router"):
+        m = int(np.ceil(0.25 * T - 1e-9))
+        assert trig.sum() >= m
+        sb = r["sigma_bar"][0].cpu().numpy()
+        assert np.array_equal(trig, sb <= np.sort(sb)[m - 1])
+        big = tt + 1 >= 2 * k                       # Eq.15 closed form on tiles that can expand fully
+        qprime = trig[big].mean()
+        assert abs(kvc[0, big].mean() - k * (1 + qprime)) < 1e-9
