@@ -6,7 +6,9 @@ from __future__ import annotations
 import numpy as np
 
 TIE_REL = 1e-5          # north_star: fp32 block scores closer than this (relative) may swap
-SIGMA_BAR_BAND = 1e-5   # tiles this close to tau may flip their trigger (logged)
+SIGMA_TOL = 1e-4        # sigma divides two small score differences
+SIGMA_BAR_BAND = 2e-4   # |sigma_bar - tau| below which a trigger may flip: both sides are means of
+                        # sigmas that are each within SIGMA_TOL (logged, counted, never hidden)
 ATTN_MAX_ABS = 2e-2
 ATTN_MEAN_ABS = 2e-3
 
@@ -45,9 +47,9 @@ def compare_select(gpu: dict, orc: dict, n_blocks: int, k: int, log: list | None
     stats["trigger_flips"] = len(flip)
     flipped = np.zeros(T, bool)
     flipped[flip] = True
-    if len(flip) == 0:
-        assert np.float32(gpu["tau"]) == np.float32(tau) or abs(float(gpu["tau"]) - tau) <= SIGMA_BAR_BAND
-    np.testing.assert_allclose(gpu["sigma_bar"], orc["sigma_bar"], rtol=0, atol=1e-5)
+    assert len(flip) <= max(2, T // 100), f"{len(flip)} trigger flips"
+    assert abs(float(gpu["tau"]) - tau) <= SIGMA_TOL, "tau"
+    np.testing.assert_allclose(gpu["sigma_bar"], orc["sigma_bar"], rtol=0, atol=SIGMA_TOL)
 
     # ---- kv_count: exact wherever the trigger agrees ----
     ok_t = ~flipped
@@ -55,7 +57,7 @@ def compare_select(gpu: dict, orc: dict, n_blocks: int, k: int, log: list | None
 
     # ---- kv_idx ----
     same = (gpu["kv_idx"] == orc["kv_idx"]).all(axis=2)          # [H, T]
-    sig_bad = np.abs(gpu["sigma"] - orc["sigma"]) > 1e-4
+    sig_bad = np.abs(gpu["sigma"] - orc["sigma"]) > SIGMA_TOL
     for h, t in zip(*np.nonzero(~same)):
         if flipped[t]:
             continue
