@@ -1,0 +1,439 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the selection + sparse-attention prefill path.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2|C3a|C3b|C4|C5|C1]
+                    [--policy router_quest] [--q-frac 0.25] [--no-extra] [--impl reference]
+
+A step is one pass of the whole hot path over one synthetic prefill layer:
+bsa_build_block_meta -> bsa_select -> bsa_sparse_attn_fwd (rows 1-6, the "sparse prefill attention")
+and bsa_dense_attn_fwd (row 7, the "x dense" denominator).  Each stage is bracketed by CUDA events on
+the launching stream; L2 is flushed (512 MiB memset) before every step, outside the event pairs.
+
+  value        = ms of rows 1-6 (pool + select + sparse attention), mean over the K timed steps,
+                 inputs resident in HBM
+  ms_per_step  = rows 1-7 (value + dense kernel)
+  x_dense      = value / dense ms (the paper's "x dense wall time", attention only)
+  e2e          = the same rows 1-6 through the C ABI from pinned HOST buffers: H2D of Q, K, V and D2H of
+                 O inside the timed region
+  roofline     = the sparse attention kernel (dominant kernel of rows 1-6) against the measured bf16 peak
+  cpu_baseline = the CPU oracle (oracle/), timed on this host's cores on a stratified 1/16 sample of the
+                 (tile, head) problems of the same workload, scaled to the full workload
+
+N > 1: the path does not shard (replicas only); every rank runs an independent
+replica, the time is the max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "sparse prefill attention ms (pool+select+sparse attn); x dense"
+PEAKS_FALLBACK = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        d["_source"] = "measured"
+        return d
+    d = dict(PEAKS_FALLBACK)
+    d["_source"] = "fallback"
+    return d
+
+
+# ---- clocks ---------------------------------------------------------------------------------------
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self._stop, self._th = index, [], threading.Event(), None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True,
+                                     timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([x.strip() for x in out.splitlines()[0].split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def start(self):
+        self._th = threading.Thread(target=self._run, daemon=True)
+        self._th.start()
+
+    def stop(self) -> dict:
+        self._stop.set()
+        if self._th:
+            self._th.join(timeout=6)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for nm, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ---- algorithmic work -----------------------------------------------------------------------------
+def algorithmic(cfg, kv_count_sum: int):
+    Bn, d, T, H = cfg.block, cfg.head_dim, cfg.n_blocks, cfg.n_q_heads
+    return {
+        "sparse_flops": 4.0 * Bn * Bn * d * kv_count_sum,               # diagonal block counted in full
+        "dense_flops": 4.0 * Bn * Bn * d * H * (T * (T + 1) / 2.0),
+        "pool_bytes": cfg.seqlen * cfg.n_kv_heads * d * 2.0,             # K read once
+    }
+
+
+# ---- the CPU oracle legs --------------------------------------------------------------------------
+def oracle_sample_ms(cfg, inp, policy: str, q_frac: float, stride: int = 16):
+    """Oracle rows 1-6 on a stratified 1/stride sample of tiles (all heads), scaled by `stride`.
+    Pooling is run in full.  Returns (ms scaled to the full workload, seconds of CPU work, sample text)."""
+    import oracle
+    oracle.max_threads()                       # builds / loads the oracle library outside the timed part
+    T, H = cfg.n_blocks, cfg.n_q_heads
+    stride = min(stride, max(T // 2, 1))
+    tiles = np.arange(stride // 2, T, stride)
+    t0 = time.perf_counter()
+    meta = oracle.pool(inp.K, cfg.block)
+    t1 = time.perf_counter()
+    r = oracle.select_tiles(inp.Q, meta, cfg.block, policy, cfg.k_budget, tiles)
+    # routing of the sampled tiles (the threshold needs every tile; on the sample it is the sample's own
+    # quantile, which keeps the triggered fraction -- and therefore the attention work -- representative)
+    sigma_bar, tau, trig = oracle.route(r["sigma"], policy, q_frac)
+    W = oracle.kv_width(policy, cfg.k_budget)
+    k = cfg.k_budget
+    n = len(tiles)
+    kv_idx = np.full((H, T, W), T, np.int32)
+    kv_count = np.zeros((H, T), np.int32)
+    for i, t in enumerate(tiles):
+        cnt = min(2 * k if trig[i] else k, t + 1)
+        kv_idx[:, t, :cnt] = r["idx_sorted"][i, :, :cnt]
+        kv_count[:, t] = cnt
+    t2 = time.perf_counter()
+    pairs = [(int(t), h) for t in tiles for h in range(H)]
+    oracle.attn_pairs(inp.Q, inp.K, inp.V, cfg.block, pairs, kv_idx, kv_count, want_lse=False)
+    t3 = time.perf_counter()
+    scaled = (t1 - t0) + (t3 - t1) * (T / n)
+    text = (f"pooling in full; scoring+top-k+sigma+routing+fill and sparse attention on {n} of {T} tiles "
+            f"(every {stride}th, all {H} heads), time scaled by {T / n:.3g}")
+    return scaled * 1e3, (t3 - t0), text
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle as it stands, on the host cores, same config / metric."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    from paper_2607_07724_b200 import synth
+    cfg = synth.CONFIGS[args.workload]
+    inp = synth.make_inputs(cfg)
+    oracle.build()
+    stride = 64 if cfg.seqlen >= 32768 else 4          # keeps warmup+steps within a few minutes
+    times = []
+    for i in range(args.warmup + args.steps):
+        ms, _, text = oracle_sample_ms(cfg, inp, args.policy, args.q_frac, stride)
+        if i >= args.warmup:
+            times.append(ms)
+    v = float(np.mean(times))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": v, "unit": "ms", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": v, "higher_is_better": False,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64 accumulate, f32 results (CPU oracle)",
+        "data": "synthetic",
+        "config": workload_config(cfg, args),
+        "cpu_baseline": {"value": v, "unit": "ms", "cores": oracle.max_threads(), "kind": "oracle",
+                         "sample": text},
+        "e2e": {"value": v, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(cfg, args):
+    return {"workload": f"{cfg.name}: B1 N={cfg.seqlen} Hq={cfg.n_q_heads} Hkv={cfg.n_kv_heads} "
+                        f"d={cfg.head_dim} block={cfg.block} k_budget={cfg.k_budget}",
+            "policy": args.policy, "q_frac": args.q_frac, "k_budget": cfg.k_budget, "seqlen": cfg.seqlen,
+            "l2": "flushed before every step (512 MiB memset outside the event pairs); "
+                  "Q+K+V+O also exceed the 126 MB L2",
+            "parallelism": "replicas only"}
+
+
+# ---- the GPU arm ----------------------------------------------------------------------------------
+class Runner:
+    """Device tensors + preallocated outputs for one workload; step() enqueues rows 1-7."""
+
+    def __init__(self, cfg, inp, policy, q_frac, torch, bsa):
+        self.cfg, self.policy, self.q_frac, self.torch, self.bsa = cfg, policy, q_frac, torch, bsa
+
+        def host(bits):
+            t = torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).view(torch.bfloat16)[None]
+            return t.pin_memory()
+
+        self.hQ, self.hK, self.hV = host(inp.Q), host(inp.K), host(inp.V)
+        self.Q, self.K, self.V = (x.cuda() for x in (self.hQ, self.hK, self.hV))
+        self.O = torch.empty_like(self.Q)
+        self.Od = torch.empty_like(self.Q)
+        self.hO = torch.empty(self.Q.shape, dtype=torch.bfloat16).pin_memory()
+        shape = bsa.make_shape(self.Q, self.K, cfg.block)
+        self.meta = torch.empty(bsa.bsa_block_meta_bytes(shape, 3), dtype=torch.uint8, device="cuda")
+        B, H, N, _ = self.Q.shape
+        T, W = cfg.n_blocks, bsa.bsa_kv_width(policy, cfg.k_budget)
+        dev = "cuda"
+        self.sel = dict(kv_idx=torch.empty((B, H, T, W), dtype=torch.int32, device=dev),
+                        kv_count=torch.empty((B, H, T), dtype=torch.int32, device=dev),
+                        sigma=torch.empty((B, H, T), dtype=torch.float32, device=dev),
+                        sigma_bar=torch.empty((B, T), dtype=torch.float32, device=dev),
+                        trigger=torch.empty((B, T), dtype=torch.uint8, device=dev),
+                        tau=torch.empty((B,), dtype=torch.float32, device=dev))
+        self.kinds = 2 if policy in ("quest", "router_quest") else 1
+        self.flush_buf = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+
+    def flush_l2(self):
+        self.flush_buf.zero_()
+
+    def sparse_path(self, Q=None, K=None, V=None, ev=None):
+        """rows 1-6; ev = list that receives events after each stage"""
+        bsa, cfg, torch = self.bsa, self.cfg, self.torch
+        Q = self.Q if Q is None else Q
+        K = self.K if K is None else K
+        V = self.V if V is None else V
+
+        def mark():
+            if ev is not None:
+                e = torch.cuda.Event(enable_timing=True)
+                e.record()
+                ev.append(e)
+        mark()
+        bsa.bsa_build_block_meta(K, cfg.block, self.kinds, self.meta)
+        mark()
+        bsa.bsa_select(Q, self.meta, K, cfg.block, self.policy, cfg.k_budget, self.q_frac, out=self.sel)
+        mark()
+        bsa.bsa_sparse_attn_fwd(Q, K, V, self.sel["kv_idx"], self.sel["kv_count"], cfg.block, O=self.O)
+        mark()
+
+    def dense(self, ev=None):
+        self.bsa.bsa_dense_attn_fwd(self.Q, self.K, self.V, self.cfg.block, O=self.Od)
+        if ev is not None:
+            e = self.torch.cuda.Event(enable_timing=True)
+            e.record()
+            ev.append(e)
+
+    def timed_steps(self, steps, warmup, with_dense=True):
+        """Returns per-stage mean ms over `steps` steps: pool, select, sparse, dense."""
+        torch = self.torch
+        for _ in range(warmup):
+            self.flush_l2()
+            self.sparse_path()
+            if with_dense:
+                self.dense()
+        torch.cuda.synchronize()
+        all_ev = []
+        for _ in range(steps):
+            self.flush_l2()
+            ev = []
+            self.sparse_path(ev=ev)
+            if with_dense:
+                self.dense(ev=ev)
+            all_ev.append(ev)
+        torch.cuda.synchronize()
+        names = ["pool", "select", "sparse"] + (["dense"] if with_dense else [])
+        per = {n: [] for n in names}
+        for ev in all_ev:
+            for i, n in enumerate(names):
+                per[n].append(ev[i].elapsed_time(ev[i + 1]))
+        return {n: float(np.mean(v)) for n, v in per.items()}, {n: float(np.min(v)) for n, v in per.items()}
+
+    def e2e_steps(self, steps, warmup):
+        """rows 1-6 from pinned host buffers: H2D Q,K,V + kernels + D2H O inside the timed region."""
+        torch = self.torch
+        times = []
+        for i in range(warmup + steps):
+            self.flush_l2()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            self.Q.copy_(self.hQ, non_blocking=True)
+            self.K.copy_(self.hK, non_blocking=True)
+            self.V.copy_(self.hV, non_blocking=True)
+            self.sparse_path()
+            self.hO.copy_(self.O, non_blocking=True)
+            e1.record()
+            torch.cuda.synchronize()
+            if i >= warmup:
+                times.append(e0.elapsed_time(e1))
+        h2d = sum(x.numel() * 2 for x in (self.hQ, self.hK, self.hV))
+        d2h = self.hO.numel() * 2
+        return float(np.mean(times)), h2d, d2h
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2607_07724_b200 import binding as bsa
+    from paper_2607_07724_b200 import synth
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback exists)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    bsa.load_library()     # raises if libbsa.so cannot be built / loaded
+    peaks = load_peaks()
+
+    cfg = synth.CONFIGS[args.workload]
+    inp = synth.make_inputs(cfg)
+    run = Runner(cfg, inp, args.policy, args.q_frac, torch, bsa)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    clocks = ClockSampler(local)
+    barrier()
+    clocks.start()
+    t_wall0 = time.perf_counter()
+    mean, best = run.timed_steps(args.steps, args.warmup)
+    barrier()
+    wall_ms = (time.perf_counter() - t_wall0) * 1e3
+    clk = clocks.stop()
+
+    sparse_ms = mean["pool"] + mean["select"] + mean["sparse"]
+    step_ms = sparse_ms + mean["dense"]
+    if world > 1:
+        t = torch.tensor([sparse_ms, step_ms, mean["sparse"], mean["dense"]], device="cuda",
+                         dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        sparse_ms, step_ms = float(t[0]), float(t[1])
+
+    kv_sum = int(run.sel["kv_count"].sum().item())
+    alg = algorithmic(cfg, kv_sum)
+    e2e_ms, h2d, d2h = run.e2e_steps(max(2, min(args.steps, 5)), 2)
+    if world > 1:
+        t = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t[0])
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    tf_sparse = alg["sparse_flops"] / (mean["sparse"] * 1e-3) / 1e12
+    tf_dense = alg["dense_flops"] / (mean["dense"] * 1e-3) / 1e12
+    pool_gbs = alg["pool_bytes"] / (mean["pool"] * 1e-3) / 1e9
+    peak_tf = peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"])
+    line = {
+        "metric": METRIC, "value": sparse_ms, "unit": "ms", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": False, "scaling": "weak",
+        "vs_baseline": None, "dtype": "bf16 (fp32 accumulate / softmax; fp32 block scores)",
+        "data": "synthetic",
+        "config": workload_config(cfg, args),
+        "tokens_per_s": cfg.seqlen * world / (sparse_ms * 1e-3),
+        "x_dense": sparse_ms / mean["dense"],
+        "x_dense_kernel_only": mean["sparse"] / mean["dense"],
+        "stages_ms": {"pool": mean["pool"], "select": mean["select"], "sparse_attn": mean["sparse"],
+                      "dense_attn": mean["dense"]},
+        "stages_ms_min": {"pool": best["pool"], "select": best["select"], "sparse_attn": best["sparse"],
+                          "dense_attn": best["dense"]},
+        "wall_ms_timed_region": wall_ms,
+        "kv_count_sum": kv_sum,
+        "mean_blocks_per_tile": kv_sum / (cfg.n_q_heads * cfg.n_blocks),
+        "roofline": {"bound": "tensor", "kernel": "attn_kernel<sparse> (bsa_sparse_attn_fwd)",
+                     "achieved": tf_sparse, "peak": peak_tf, "unit": "TFLOP/s", "frac": tf_sparse / peak_tf,
+                     "traffic": None, "peak_source": f"{peaks['_source']} bf16_tflops_sustained",
+                     "algorithmic_flops_per_launch": alg["sparse_flops"]},
+        "roofline_dense": {"bound": "tensor", "achieved": tf_dense, "peak": peak_tf, "unit": "TFLOP/s",
+                           "frac": tf_dense / peak_tf},
+        "roofline_pool": {"bound": "hbm", "achieved": pool_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                          "frac": pool_gbs / peaks["hbm_gbs"], "algorithmic_bytes": alg["pool_bytes"],
+                          "note": "cold L2 (flushed before the step)"},
+        "e2e": {"value": e2e_ms, "unit": "ms", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+        "gpu_launches": (args.steps) * (5 if args.policy.startswith("router") else 4)
+                        + args.steps,     # + the dense kernel of every step
+        "clocks": clk,
+    }
+
+    # ---- the long-context ratio regime (BASELINE.json configs[2]): 64K / 128K, few steps ------------
+    if not args.no_extra and args.workload == "C2" and world == 1:
+        extra = {}
+        del run
+        torch.cuda.empty_cache()
+        for name in ("C3a", "C3b"):
+            c = synth.CONFIGS[name]
+            i2 = synth.make_inputs(c)
+            for pol in ("router_quest", "topk"):
+                r2 = Runner(c, i2, pol, args.q_frac, torch, bsa)
+                m2, _ = r2.timed_steps(3, 1, with_dense=(pol == "router_quest"))
+                if pol == "router_quest":
+                    dense_ms = m2["dense"]
+                s = m2["pool"] + m2["select"] + m2["sparse"]
+                kvs = int(r2.sel["kv_count"].sum().item())
+                a2 = algorithmic(c, kvs)
+                extra[f"{name}/{pol}"] = {
+                    "seqlen": c.seqlen, "sparse_path_ms": s, "pool_ms": m2["pool"], "select_ms": m2["select"],
+                    "sparse_attn_ms": m2["sparse"], "dense_attn_ms": dense_ms, "x_dense": s / dense_ms,
+                    "sparse_tflops": a2["sparse_flops"] / (m2["sparse"] * 1e-3) / 1e12,
+                    "dense_tflops": a2["dense_flops"] / (dense_ms * 1e-3) / 1e12}
+                del r2
+                torch.cuda.empty_cache()
+        line["long_context"] = extra
+
+    # ---- CPU oracle on this host's cores --------------------------------------------------------------
+    import oracle
+    cpu_ms, cpu_s, text = oracle_sample_ms(cfg, inp, args.policy, args.q_frac, 16)
+    line["cpu_baseline"] = {"value": cpu_ms, "unit": "ms", "cores": oracle.max_threads(), "kind": "oracle",
+                            "sample": text, "cpu_seconds_spent": cpu_s}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="C2")
+    ap.add_argument("--policy", default="router_quest")
+    ap.add_argument("--q-frac", type=float, default=0.25)
+    ap.add_argument("--impl", default="bsa", choices=["bsa", "reference"])
+    ap.add_argument("--no-extra", action="store_true", help="skip the 64K / 128K ratio runs")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()
