@@ -15,7 +15,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libbsa.so")
-SOURCES = ["api.cu", "pool.cu", "select.cu", "attn.cu"]
+SOURCES = ["api.cu", "pool.cu", "select.cu", "score_tc.cu", "attn.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 

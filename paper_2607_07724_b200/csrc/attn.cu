@@ -16,6 +16,7 @@
 
 #include "bsa_internal.h"
 #include "sm100_ptx.cuh"
+#include "tmap.h"
 
 namespace bsa {
 
@@ -325,51 +326,14 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
 }
 
 // ---- host side ---------------------------------------------------------------------------------
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
-                                  const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
-                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-EncodeTiledFn encode_fn() {
-  static EncodeTiledFn fn = nullptr;
-  if (!fn) {
-    void* p = nullptr;
-    cudaDriverEntryPointQueryResult q;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
-        q == cudaDriverEntryPointSuccess)
-      fn = reinterpret_cast<EncodeTiledFn>(p);
-  }
-  return fn;
-}
-
-// bf16 tensor [B, heads, N, d] (strides in elements) viewed as 5-D (64, N, d/64, heads, B) so one
-// TMA instruction lands a [rows x d] tile as d/64 consecutive 128B-swizzled [rows x 64] chunks.
-bool make_tmap(CUtensorMap* m, const void* base, int B, int heads, int N, int d, int64_t sb,
-               int64_t sh, int64_t sn, int rows) {
-  EncodeTiledFn fn = encode_fn();
-  if (!fn) return false;
-  cuuint64_t dims[5] = {64, static_cast<cuuint64_t>(N), static_cast<cuuint64_t>(d / 64),
-                        static_cast<cuuint64_t>(heads), static_cast<cuuint64_t>(B)};
-  cuuint64_t strides[4] = {static_cast<cuuint64_t>(sn) * 2, 128, static_cast<cuuint64_t>(sh) * 2,
-                           static_cast<cuuint64_t>(sb) * 2};
-  if (heads == 1) strides[2] = strides[0] * static_cast<cuuint64_t>(N);
-  if (B == 1) strides[3] = strides[2] * static_cast<cuuint64_t>(heads);
-  cuuint32_t box[5] = {64, static_cast<cuuint32_t>(rows), static_cast<cuuint32_t>(d / 64), 1, 1};
-  cuuint32_t es[5] = {1, 1, 1, 1, 1};
-  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 5, const_cast<void*>(base), dims, strides, box,
-                  es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
-                  CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  return r == CUDA_SUCCESS;
-}
-
 template <int BM, int D, bool SPARSE>
 bsa_status run(const Dims& S, const void* Q, const void* K, const void* V, const Params& prm,
                cudaStream_t stream) {
   using C = Cfg<BM, D>;
   CUtensorMap tq, tk, tv;
-  if (!make_tmap(&tq, Q, S.B, S.H, S.N, S.d, S.qsb, S.qsh, S.qsn, BM) ||
-      !make_tmap(&tk, K, S.B, S.Hkv, S.N, S.d, S.ksb, S.ksh, S.ksn, BN) ||
-      !make_tmap(&tv, V, S.B, S.Hkv, S.N, S.d, S.ksb, S.ksh, S.ksn, BN))
+  if (!make_tmap_bhnd(&tq, Q, S.B, S.H, S.N, S.d, S.qsb, S.qsh, S.qsn, BM, S.d / 64, 1) ||
+      !make_tmap_bhnd(&tk, K, S.B, S.Hkv, S.N, S.d, S.ksb, S.ksh, S.ksn, BN, S.d / 64, 1) ||
+      !make_tmap_bhnd(&tv, V, S.B, S.Hkv, S.N, S.d, S.ksb, S.ksh, S.ksn, BN, S.d / 64, 1))
     return fail(BSA_ERR_CUDA, "attn: cuTensorMapEncodeTiled failed");
   auto kern = attn_kernel<BM, D, SPARSE>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM);

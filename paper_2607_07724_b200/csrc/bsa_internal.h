@@ -36,6 +36,11 @@ bsa_status launch_pool(const Dims& D, const void* K, int kinds, void* meta, cuda
 bsa_status launch_select(const Dims& D, const void* Q, const void* meta, int policy, int k, int W,
                          long long m_route, int32_t* kv_idx, int32_t* kv_count, float* sigma,
                          float* sigma_bar, uint8_t* trigger, float* tau, cudaStream_t stream);
+// tensor-core scoring + tile max + top-(2k) + sigma (score_tc.cu); writes kv_idx (all 2k/k slots),
+// sigma and, for the non-router policies, kv_count.
+bsa_status launch_score_tc(const Dims& D, const void* Q, const void* meta, bool quest, int k, int W,
+                           int router, int32_t* kv_idx, int32_t* kv_count, float* sigma,
+                           cudaStream_t stream);
 bsa_status launch_attn(const Dims& D, const void* Q, const void* K, const void* V,
                        const int32_t* kv_idx, const int32_t* kv_count, int W, bool sparse,
                        float scale, void* O, float* lse, cudaStream_t stream);

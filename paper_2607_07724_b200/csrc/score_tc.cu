@@ -1,0 +1,298 @@
+// score_tc.cu -- tensor-core block scoring fused with tile-max, top-(2k) and sigma
+// (Eq.1-4; A.2-A.6 L296-324; readings G1, G4-G8 in DESIGN.md).
+//
+// One CTA per (tile t, KV head g, head set) where a head set is up to NH query heads of the GQA
+// group.  The product is computed TRANSPOSED so that the tile max (Eq.3) is a per-thread loop:
+//     S^T[block, (head, row)] = Pooled[block, :] . Qplanes[(head, row), :]
+//   A (M = 128 pooled blocks, K-major)  streamed by TMA from the meta planes through a ring,
+//   B (N = heads*BN query rows)         resident in shared memory,
+//   D in TMEM, double buffered: lanes = blocks, columns = query rows.
+// Quest (Eq.2):  sum_c max(q_c Kmax_c, q_c Kmin_c) = q+ . Kmax + q- . Kmin with q+ = max(q,0),
+//   q- = min(q,0); all four operands are bf16-exact, K dimension 2d.
+// K-mean (Eq.1): kmean (fp32) = hi + mid + lo exactly (three bf16 planes written by the pooling
+//   kernel), K dimension 3d against the same Q chunk; products are exact, accumulation is fp32.
+// Warps 0-3: Q+/Q- conversion, epilogue (column max per head -> shared-memory score rows), then one
+//   warp per head runs warp_select (select_common.cuh).   Warp 4: TMA producer.   Warp 5: MMA issue.
+#include <cuda_bf16.h>
+
+#include "bsa_internal.h"
+#include "select_common.cuh"
+#include "sm100_ptx.cuh"
+#include "tmap.h"
+
+namespace bsa {
+
+namespace {
+
+constexpr int kTcThreads = 192;
+constexpr int kABlocks = 128;                 // pooled blocks per MMA (UMMA M)
+constexpr int kAStageBytes = kABlocks * 128;  // one [128 blocks x 64 elem] swizzled tile
+constexpr int kMaxStages = 6;
+
+template <int D, int BN, bool QUEST>
+struct TcCfg {
+  static constexpr int PLANES_B = QUEST ? 2 : 1;          // q+ | q-   or   q
+  static constexpr int PLANES_A = QUEST ? 2 : 3;          // kmax | kmin   or   hi | mid | lo
+  static constexpr int DC = D / 64;                        // 64-element K chunks per plane
+  static constexpr int HEAD_B_BYTES = BN * D * 2 * PLANES_B;
+  static constexpr int NH_N = 256 / BN;                    // UMMA N <= 256
+  static constexpr int NH_S = (128 * 1024) / HEAD_B_BYTES; // B planes <= 128 KB
+  static constexpr int NH = NH_N < NH_S ? NH_N : NH_S;
+  static constexpr int NROWS = NH * BN;                    // rows of one B chunk tile
+  static constexpr int B_CHUNK_BYTES = NROWS * 128;
+  static constexpr int B_BYTES = B_CHUNK_BYTES * DC * PLANES_B;
+  static constexpr int KCHUNKS = PLANES_A * DC;            // A chunks per block chunk
+  static constexpr uint32_t TMEM_COLS = (2 * NROWS <= 32) ? 32 : (2 * NROWS <= 64) ? 64
+                                        : (2 * NROWS <= 128) ? 128 : (2 * NROWS <= 256) ? 256 : 512;
+  static_assert(NH >= 1, "B planes of one head do not fit");
+};
+
+struct TcParams {
+  int32_t* kv_idx;
+  int32_t* kv_count;
+  float* sigma;
+  int B, H, Hkv, G, NB, k, W, router, sets, stages, nbpad;
+  float inv_sqrt_d;
+};
+
+struct alignas(8) TcCtl {
+  uint64_t q_full, b_ready;
+  uint64_t a_full[kMaxStages], a_empty[kMaxStages];
+  uint64_t acc_full[2], acc_empty[2];
+  uint32_t tmem_base;
+};
+
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+template <int D, int BN, bool QUEST>
+__global__ void __launch_bounds__(kTcThreads, 1)
+score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmA,
+                const TcParams p) {
+  using C = TcCfg<D, BN, QUEST>;
+  extern __shared__ __align__(1024) uint8_t smem[];
+  uint8_t* b_s = smem;                                   // [PLANES_B][DC][NROWS x 128 B]
+  uint8_t* a_s = smem + C::B_BYTES;                      // ring of [128 x 128 B] stages
+  float* sc = reinterpret_cast<float*>(a_s + p.stages * kAStageBytes);      // [NH][nbpad]
+  unsigned long long* cand = reinterpret_cast<unsigned long long*>(sc + C::NH * p.nbpad);
+  TcCtl* ctl = reinterpret_cast<TcCtl*>(cand + C::NH * kMaxCand);
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  // unit: heaviest tiles first
+  const int per_tile = p.B * p.Hkv * p.sets;
+  const int t = p.NB - 1 - static_cast<int>(blockIdx.x) / per_tile;
+  int rem = static_cast<int>(blockIdx.x) % per_tile;
+  const int b = rem / (p.Hkv * p.sets);
+  rem %= p.Hkv * p.sets;
+  const int g = rem / p.sets, set = rem % p.sets;
+  const int h0 = g * p.G + set * C::NH;
+  const int nh = (p.G - set * C::NH) < C::NH ? (p.G - set * C::NH) : C::NH;   // heads in this set
+  const int n_chunks = (t + 1 + kABlocks - 1) / kABlocks;
+
+  if ((smem_u32(smem) & 1023u) != 0) __trap();
+
+  if (warp == 5 && lane == 0) {
+    mbar_init(smem_u32(&ctl->q_full), 1);
+    mbar_init(smem_u32(&ctl->b_ready), 4);
+    for (int s = 0; s < p.stages; ++s) {
+      mbar_init(smem_u32(&ctl->a_full[s]), 1);
+      mbar_init(smem_u32(&ctl->a_empty[s]), 1);
+    }
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(smem_u32(&ctl->acc_full[i]), 1);
+      mbar_init(smem_u32(&ctl->acc_empty[i]), 4);
+    }
+    fence_mbar_init();
+  }
+  if (warp == 4) {
+    if (lane == 0) {
+      tma_prefetch_desc(&tmQ);
+      tma_prefetch_desc(&tmA);
+    }
+    __syncwarp();
+    tmem_alloc<C::TMEM_COLS>(smem_u32(&ctl->tmem_base));
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = ctl->tmem_base;
+
+  if (warp == 4) {
+    // ---- TMA producer ------------------------------------------------------------------------
+    if (lane == 0) {
+      mbar_arrive_expect_tx(smem_u32(&ctl->q_full), C::DC * C::B_CHUNK_BYTES);
+      for (int c64 = 0; c64 < C::DC; ++c64)
+        tma_load_5d(smem_u32(b_s + c64 * C::B_CHUNK_BYTES), &tmQ, smem_u32(&ctl->q_full), 0, t * BN,
+                    c64, h0, b);
+      int it = 0;
+      for (int c = 0; c < n_chunks; ++c) {
+        for (int kc = 0; kc < C::KCHUNKS; ++kc, ++it) {
+          const int s = it % p.stages;
+          const int pa = kc / C::DC, c64 = kc % C::DC;
+          const int mem_plane = QUEST ? (1 - pa) : pa;   // memory order: [kmin, kmax] / [hi, mid, lo]
+          mbar_wait(smem_u32(&ctl->a_empty[s]), ((it / p.stages) & 1) ^ 1);
+          mbar_arrive_expect_tx(smem_u32(&ctl->a_full[s]), kAStageBytes);
+          tma_load_5d(smem_u32(a_s + s * kAStageBytes), &tmA, smem_u32(&ctl->a_full[s]), c64 * 64,
+                      c * kABlocks, g, b, mem_plane);
+        }
+      }
+    }
+  } else if (warp == 5) {
+    // ---- MMA issuer --------------------------------------------------------------------------
+    if (lane == 0) {
+      const uint32_t idesc = umma_idesc_bf16(kABlocks, nh * BN, 0, 0);
+      const uint32_t b_a = smem_u32(b_s), a_a = smem_u32(a_s);
+      mbar_wait(smem_u32(&ctl->b_ready), 0);
+      tc_fence_after();
+      int it = 0;
+      for (int c = 0; c < n_chunks; ++c) {
+        const int buf = c & 1;
+        if (c >= 2) {
+          mbar_wait(smem_u32(&ctl->acc_empty[buf]), ((c >> 1) & 1) ^ 1);
+          tc_fence_after();
+        }
+        const uint32_t tD = tmem + buf * C::NROWS;
+        for (int kc = 0; kc < C::KCHUNKS; ++kc, ++it) {
+          const int s = it % p.stages;
+          const int bchunk = QUEST ? kc : (kc % C::DC);
+          mbar_wait(smem_u32(&ctl->a_full[s]), (it / p.stages) & 1);
+          tc_fence_after();
+#pragma unroll
+          for (int ks = 0; ks < 4; ++ks) {
+            const uint64_t ad = umma_smem_desc(a_a + s * kAStageBytes + ks * 32, 16, 1024);
+            const uint64_t bd = umma_smem_desc(b_a + bchunk * C::B_CHUNK_BYTES + ks * 32, 16, 1024);
+            umma_ss(tD, ad, bd, idesc, (kc > 0) || (ks > 0));
+          }
+          tc_commit(smem_u32(&ctl->a_empty[s]));
+        }
+        tc_commit(smem_u32(&ctl->acc_full[buf]));
+      }
+    }
+  } else {
+    // ---- conversion, epilogue, selection (warps 0-3) -----------------------------------------
+    mbar_wait(smem_u32(&ctl->q_full), 0);
+    if (QUEST) {
+      // q+ = max(q, 0) in place, q- = min(q, 0) into plane 1 (element-wise, swizzle preserved)
+      constexpr int PLANE = C::DC * C::B_CHUNK_BYTES;
+      for (int i = tid; i < PLANE / 16; i += 128) {
+        uint4 v = *reinterpret_cast<uint4*>(b_s + i * 16);
+        uint32_t w[4] = {v.x, v.y, v.z, v.w}, pos[4], neg[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const uint32_t nm = ((w[j] & 0x80008000u) >> 15) * 0xFFFFu;  // 0xFFFF per negative half
+          neg[j] = w[j] & nm;
+          pos[j] = w[j] & ~nm;
+        }
+        *reinterpret_cast<uint4*>(b_s + i * 16) = make_uint4(pos[0], pos[1], pos[2], pos[3]);
+        *reinterpret_cast<uint4*>(b_s + PLANE + i * 16) = make_uint4(neg[0], neg[1], neg[2], neg[3]);
+      }
+      fence_proxy_async_smem();
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(smem_u32(&ctl->b_ready));
+
+    const uint32_t lane_base = static_cast<uint32_t>(warp * 32) << 16;
+    for (int c = 0; c < n_chunks; ++c) {
+      const int buf = c & 1;
+      mbar_wait(smem_u32(&ctl->acc_full[buf]), (c >> 1) & 1);
+      tc_fence_after();
+      const int blk = c * kABlocks + warp * 32 + lane;
+      const uint32_t tD = tmem + lane_base + buf * C::NROWS;
+      for (int j = 0; j < nh; ++j) {
+        float mx = -INFINITY;
+#pragma unroll
+        for (int c0 = 0; c0 < BN; c0 += 64) {
+          uint32_t ra[32], rb[32];
+          tmem_ld32(tD + j * BN + c0, ra);
+          tmem_ld32(tD + j * BN + c0 + 32, rb);
+          tmem_ld_wait();
+#pragma unroll
+          for (int i = 0; i < 32; ++i)
+            mx = fmaxf(mx, fmaxf(__uint_as_float(ra[i]), __uint_as_float(rb[i])));
+        }
+        if (blk <= t) sc[j * p.nbpad + blk] = QUEST ? mx : mx * p.inv_sqrt_d;   // Eq.3 (G8)
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(smem_u32(&ctl->acc_empty[buf]));
+    }
+    named_bar_sync(1, 128);
+    if (warp < nh) {
+      const int h = h0 + warp;
+      const int64_t row = (static_cast<int64_t>(b) * p.H + h) * p.NB + t;
+      const float sig = warp_select(sc + warp * p.nbpad, t, p.k, p.NB, p.W, p.kv_idx + row * p.W,
+                                    cand + warp * kMaxCand, lane);
+      if (lane == 0) {
+        p.sigma[row] = sig;
+        if (!p.router) p.kv_count[row] = (p.k < t + 1) ? p.k : t + 1;
+      }
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 4) tmem_dealloc<C::TMEM_COLS>(tmem);
+}
+
+template <int D, int BN, bool QUEST>
+bsa_status run_score_tc(const Dims& S, const void* Q, const char* meta, const MetaLayout& L, int k, int W,
+                        int router, int32_t* kv_idx, int32_t* kv_count, float* sigma,
+                        cudaStream_t stream) {
+  using C = TcCfg<D, BN, QUEST>;
+  TcParams p;
+  p.kv_idx = kv_idx; p.kv_count = kv_count; p.sigma = sigma;
+  p.B = S.B; p.H = S.H; p.Hkv = S.Hkv; p.G = S.G; p.NB = S.NB; p.k = k; p.W = W; p.router = router;
+  p.sets = (S.G + C::NH - 1) / C::NH;
+  p.nbpad = (S.NB + 3) & ~3;
+  p.inv_sqrt_d = static_cast<float>(1.0 / sqrt(static_cast<double>(S.d)));
+  const size_t fixed = static_cast<size_t>(C::B_BYTES) + static_cast<size_t>(C::NH) * p.nbpad * 4 +
+                       static_cast<size_t>(C::NH) * kMaxCand * 8 + sizeof(TcCtl);
+  const size_t budget = 227 * 1024;
+  if (fixed + 2 * kAStageBytes > budget)
+    return fail(BSA_ERR_UNSUPPORTED, "select: %d blocks per sequence need too much shared memory", S.NB);
+  int stages = static_cast<int>((budget - fixed) / kAStageBytes);
+  p.stages = stages > kMaxStages ? kMaxStages : stages;
+  const size_t smem = fixed + static_cast<size_t>(p.stages) * kAStageBytes;
+
+  CUtensorMap tq, ta;
+  if (!make_tmap_bhnd(&tq, Q, S.B, S.H, S.N, S.d, S.qsb, S.qsh, S.qsn, BN, 1, C::NH))
+    return fail(BSA_ERR_CUDA, "select: cuTensorMapEncodeTiled(Q) failed");
+  {
+    const char* base = meta + (QUEST ? L.off_min : L.off_split);
+    const cuuint64_t d2 = static_cast<cuuint64_t>(S.d) * 2;
+    cuuint64_t dims[5] = {static_cast<cuuint64_t>(S.d), static_cast<cuuint64_t>(S.NB),
+                          static_cast<cuuint64_t>(S.Hkv), static_cast<cuuint64_t>(S.B),
+                          static_cast<cuuint64_t>(C::PLANES_A)};
+    cuuint64_t strides[4] = {d2, d2 * S.NB, d2 * S.NB * S.Hkv, static_cast<cuuint64_t>(L.elems) * 2};
+    cuuint32_t box[5] = {64, kABlocks, 1, 1, 1};
+    if (!make_tmap_bf16(&ta, base, 5, dims, strides, box))
+      return fail(BSA_ERR_CUDA, "select: cuTensorMapEncodeTiled(meta) failed");
+  }
+  auto kern = score_tc_kernel<D, BN, QUEST>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       static_cast<int>(smem));
+  if (e != cudaSuccess) return fail(BSA_ERR_CUDA, "select: smem attribute: %s", cudaGetErrorString(e));
+  const long long grid = static_cast<long long>(S.NB) * S.B * S.Hkv * p.sets;
+  if (grid > 0x7fffffffLL) return fail(BSA_ERR_UNSUPPORTED, "select: grid too large");
+  kern<<<static_cast<unsigned>(grid), kTcThreads, smem, stream>>>(tq, ta, p);
+  return check_launch("score_tc_kernel");
+}
+
+}  // namespace
+
+bsa_status launch_score_tc(const Dims& S, const void* Q, const void* meta, bool quest, int k, int W,
+                           int router, int32_t* kv_idx, int32_t* kv_count, float* sigma,
+                           cudaStream_t stream) {
+  const MetaLayout L = meta_layout(S);
+  const char* mp = static_cast<const char*>(meta);
+#define BSA_TC(DD, BB)                                                                              \
+  if (S.d == DD && S.Bn == BB)                                                                      \
+    return quest ? run_score_tc<DD, BB, true>(S, Q, mp, L, k, W, router, kv_idx, kv_count, sigma, stream) \
+                 : run_score_tc<DD, BB, false>(S, Q, mp, L, k, W, router, kv_idx, kv_count, sigma, stream);
+  BSA_TC(64, 64) BSA_TC(128, 64) BSA_TC(256, 64) BSA_TC(64, 128) BSA_TC(128, 128) BSA_TC(256, 128)
+#undef BSA_TC
+  return fail(BSA_ERR_UNSUPPORTED, "select: unsupported head_dim %d / block %d", S.d, S.Bn);
+}
+
+}  // namespace bsa
