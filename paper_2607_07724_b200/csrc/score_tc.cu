@@ -60,6 +60,7 @@ struct alignas(8) TcCtl {
   uint64_t a_full[kMaxStages], a_empty[kMaxStages];
   uint64_t acc_full[2], acc_empty[2];
   uint32_t tmem_base;
+  uint32_t s3[4 * 4];   // per-warp scratch of warp_select
 };
 
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
@@ -74,7 +75,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   extern __shared__ __align__(1024) uint8_t smem[];
   uint8_t* b_s = smem;                                   // [PLANES_B][DC][NROWS x 128 B]
   uint8_t* a_s = smem + C::B_BYTES;                      // ring of [128 x 128 B] stages
-  float* sc = reinterpret_cast<float*>(a_s + p.stages * kAStageBytes);      // [NH][nbpad]
+  uint32_t* sc = reinterpret_cast<uint32_t*>(a_s + p.stages * kAStageBytes);   // [NH][nbpad] okey(score)
   unsigned long long* cand = reinterpret_cast<unsigned long long*>(sc + C::NH * p.nbpad);
   TcCtl* ctl = reinterpret_cast<TcCtl*>(cand + C::NH * kMaxCand);
 
@@ -211,7 +212,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           for (int i = 0; i < 32; ++i)
             mx = fmaxf(mx, fmaxf(__uint_as_float(ra[i]), __uint_as_float(rb[i])));
         }
-        if (blk <= t) sc[j * p.nbpad + blk] = QUEST ? mx : mx * p.inv_sqrt_d;   // Eq.3 (G8)
+        if (blk <= t) sc[j * p.nbpad + blk] = okey(QUEST ? mx : mx * p.inv_sqrt_d);   // Eq.3 (G8)
       }
       tc_fence_before();
       __syncwarp();
@@ -222,7 +223,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       const int h = h0 + warp;
       const int64_t row = (static_cast<int64_t>(b) * p.H + h) * p.NB + t;
       const float sig = warp_select(sc + warp * p.nbpad, t, p.k, p.NB, p.W, p.kv_idx + row * p.W,
-                                    cand + warp * kMaxCand, lane);
+                                    cand + warp * kMaxCand, ctl->s3 + warp * 4, lane);
       if (lane == 0) {
         p.sigma[row] = sig;
         if (!p.router) p.kv_count[row] = (p.k < t + 1) ? p.k : t + 1;
