@@ -23,7 +23,6 @@ namespace bsa {
 namespace {
 
 constexpr int BN = 64;                 // keys per pipeline stage / per S tile
-constexpr int kSoftmaxThreads = 128;
 constexpr int kThreads = 192;
 constexpr int kMaxW = 256;             // widest kv_idx row staged in shared memory
 
@@ -62,6 +61,270 @@ struct alignas(8) Ctl {
 };
 static_assert(sizeof(Ctl) <= 1024, "Ctl must fit the 1 KB bookkeeping area");
 
+// ---- softmax warps, BM = 128 (dense; sparse with 128-token blocks) -------------------------------
+// Thread r owns accumulator row r (TMEM lane r, 32x32b loads).  Logits stay unscaled in registers;
+// the softmax scale is folded into one FFMA per element: p = 2^(s*scale_log2 - m).
+template <int D, bool SPARSE, class KeyStart>
+__device__ __forceinline__ void softmax_m128(const Params& p, Ctl* ctl, uint8_t* p_s, uint32_t tmem,
+                                             int n_it, int q0, int b, int h, KeyStart key_start) {
+  using C = Cfg<128, D>;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int r = tid, qrow = q0 + r;
+  const uint32_t lane_base = static_cast<uint32_t>(warp * 32) << 16;
+  const uint32_t tS = tmem + lane_base, tO = tmem + lane_base + C::O_COL;
+  const float sc = p.scale_log2;
+  float m = -INFINITY, l = 0.f;
+  for (int j = 0; j < n_it; ++j) {
+    const int k0 = key_start(j);
+    mbar_wait(smem_u32(&ctl->s_full), j & 1);
+    tc_fence_after();
+    uint32_t sa[32], sb[32];
+    tmem_ld32(tS, sa);
+    tmem_ld32(tS + 32, sb);
+    tmem_ld_wait();
+    tc_fence_before();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(smem_u32(&ctl->s_free));
+
+    float x[64];
+#pragma unroll
+    for (int c = 0; c < 32; ++c) {
+      x[c] = __uint_as_float(sa[c]);
+      x[c + 32] = __uint_as_float(sb[c]);
+    }
+    if (k0 + BN - 1 > q0) {  // only blocks touching the diagonal need the causal mask
+#pragma unroll
+      for (int c = 0; c < 64; ++c) x[c] = (k0 + c <= qrow) ? x[c] : -INFINITY;
+    }
+    float mx = fmaxf(x[0], x[1]);
+#pragma unroll
+    for (int c = 2; c < 64; c += 2) mx = fmax3(mx, x[c], x[c + 1]);
+    float m_new = fmaxf(m, mx * sc);
+    // lazy rescale: keep the stale reference max unless some row of this warp grew by > 2^8
+    const bool any = __any_sync(0xffffffffu, m_new - m > 8.0f);
+    if (!any) m_new = m;
+    const float alpha = ex2_approx(m - m_new);
+    float sum = 0.f;
+    uint32_t pk[32];
+#pragma unroll
+    for (int c = 0; c < 64; c += 2) {
+      const float e0 = ex2_approx(fmaf(x[c], sc, -m_new)), e1 = ex2_approx(fmaf(x[c + 1], sc, -m_new));
+      sum += e0 + e1;
+      pk[c >> 1] = pack_bf16x2(e0, e1);
+    }
+    l = l * alpha + sum;
+    m = m_new;
+
+    if (j > 0) {
+      mbar_wait(smem_u32(&ctl->o_done), (j - 1) & 1);  // PV(j-1) done: P and O are ours
+      tc_fence_after();
+      if (any) {
+#pragma unroll
+        for (int c0 = 0; c0 < D; c0 += 32) {
+          uint32_t o[32];
+          tmem_ld32(tO + c0, o);
+          tmem_ld_wait();
+#pragma unroll
+          for (int c = 0; c < 32; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * alpha);
+          tmem_st32(tO + c0, o);
+        }
+        tmem_st_wait();
+      }
+    }
+    uint8_t* prow = p_s + r * 128;
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+      uint4 v = make_uint4(pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
+      *reinterpret_cast<uint4*>(prow + ((c ^ (r & 7)) << 4)) = v;
+    }
+    fence_proxy_async_smem();
+    tc_fence_before();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(smem_u32(&ctl->p_full));
+  }
+  // ---- epilogue: O / l -> bf16 -> global ---------------------------------------------------------
+  mbar_wait(smem_u32(&ctl->o_done), (n_it - 1) & 1);
+  tc_fence_after();
+  const float inv_l = 1.0f / l;
+  const bool store = qrow < p.N;
+  uint16_t* orow = p.O + b * p.qsb + h * p.qsh + static_cast<int64_t>(qrow) * p.qsn;
+#pragma unroll
+  for (int c0 = 0; c0 < D; c0 += 32) {
+    uint32_t o[32];
+    tmem_ld32(tO + c0, o);
+    tmem_ld_wait();
+    if (store) {
+#pragma unroll
+      for (int c = 0; c < 32; c += 8) {
+        uint4 v;
+        v.x = pack_bf16x2(__uint_as_float(o[c]) * inv_l, __uint_as_float(o[c + 1]) * inv_l);
+        v.y = pack_bf16x2(__uint_as_float(o[c + 2]) * inv_l, __uint_as_float(o[c + 3]) * inv_l);
+        v.z = pack_bf16x2(__uint_as_float(o[c + 4]) * inv_l, __uint_as_float(o[c + 5]) * inv_l);
+        v.w = pack_bf16x2(__uint_as_float(o[c + 6]) * inv_l, __uint_as_float(o[c + 7]) * inv_l);
+        *reinterpret_cast<uint4*>(orow + c0 + c) = v;
+      }
+    }
+  }
+  if (store && p.lse)
+    p.lse[(static_cast<int64_t>(b) * p.H + h) * p.N + qrow] = (m + log2f(l)) * 0.6931471805599453f;
+  tc_fence_before();
+}
+
+// ---- softmax warps, BM = 64 (sparse, 64-token blocks) -------------------------------------------
+// A UMMA M = 64 accumulator keeps row r in TMEM lane 32*(r/16) + r%16, i.e. only 16 of the 32 lanes
+// of each warp's quadrant.  A 32x32b load would leave half the threads idle through the whole
+// softmax; the 16x256b shape instead spreads the 16 lanes x 64 columns over all 32 threads: thread
+// t owns rows rA = 16w + t/4 and rB = rA + 8, and in every 8-column group the two columns
+// 2(t%4), 2(t%4)+1.  Row max = in-thread max + two quad shuffles; the row sum stays a per-thread
+// partial until the epilogue.
+template <int D, bool SPARSE, class KeyStart>
+__device__ __forceinline__ void softmax_m64(const Params& p, Ctl* ctl, uint8_t* p_s, uint32_t tmem,
+                                            int n_it, int q0, int b, int h, KeyStart key_start) {
+  using C = Cfg<64, D>;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int quad = lane & 3;
+  const int rA = warp * 16 + (lane >> 2), rB = rA + 8;
+  const int qrA = q0 + rA, qrB = q0 + rB;
+  const uint32_t lane_base = static_cast<uint32_t>(warp * 32) << 16;
+  const uint32_t tS = tmem + lane_base, tO = tmem + lane_base + C::O_COL;
+  const float sc = p.scale_log2;
+  float mA = -INFINITY, mB = -INFINITY, lA = 0.f, lB = 0.f;
+  uint8_t* prowA = p_s + rA * 128 + quad * 4;
+  uint8_t* prowB = p_s + rB * 128 + quad * 4;
+  const int sw = rA & 7;  // == rB & 7
+  for (int j = 0; j < n_it; ++j) {
+    const int k0 = key_start(j);
+    mbar_wait(smem_u32(&ctl->s_full), j & 1);
+    tc_fence_after();
+    uint32_t s[32];
+    tmem_ld16x256_x8(tS, s);
+    tmem_ld_wait();
+    tc_fence_before();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(smem_u32(&ctl->s_free));
+
+    float xa[16], xb[16];
+#pragma unroll
+    for (int g = 0; g < 8; ++g) {
+      xa[2 * g] = __uint_as_float(s[4 * g]);
+      xa[2 * g + 1] = __uint_as_float(s[4 * g + 1]);
+      xb[2 * g] = __uint_as_float(s[4 * g + 2]);
+      xb[2 * g + 1] = __uint_as_float(s[4 * g + 3]);
+    }
+    if (k0 + BN - 1 > q0) {
+#pragma unroll
+      for (int g = 0; g < 8; ++g) {
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const int key = k0 + 8 * g + 2 * quad + e;
+          xa[2 * g + e] = (key <= qrA) ? xa[2 * g + e] : -INFINITY;
+          xb[2 * g + e] = (key <= qrB) ? xb[2 * g + e] : -INFINITY;
+        }
+      }
+    }
+    float mxA = fmaxf(xa[0], xa[1]), mxB = fmaxf(xb[0], xb[1]);
+#pragma unroll
+    for (int c = 2; c < 16; c += 2) {
+      mxA = fmax3(mxA, xa[c], xa[c + 1]);
+      mxB = fmax3(mxB, xb[c], xb[c + 1]);
+    }
+    mxA = fmaxf(mxA, __shfl_xor_sync(0xffffffffu, mxA, 1));
+    mxB = fmaxf(mxB, __shfl_xor_sync(0xffffffffu, mxB, 1));
+    mxA = fmaxf(mxA, __shfl_xor_sync(0xffffffffu, mxA, 2));
+    mxB = fmaxf(mxB, __shfl_xor_sync(0xffffffffu, mxB, 2));
+    float mA_new = fmaxf(mA, mxA * sc), mB_new = fmaxf(mB, mxB * sc);
+    // lazy rescale: keep the stale reference maxima unless some row of this warp grew by > 2^8
+    const bool any = __any_sync(0xffffffffu, (mA_new - mA > 8.0f) || (mB_new - mB > 8.0f));
+    if (!any) {
+      mA_new = mA;
+      mB_new = mB;
+    }
+    const float alphaA = ex2_approx(mA - mA_new), alphaB = ex2_approx(mB - mB_new);
+    float sumA = 0.f, sumB = 0.f;
+    uint32_t pa[8], pb[8];
+#pragma unroll
+    for (int g = 0; g < 8; ++g) {
+      const float a0 = ex2_approx(fmaf(xa[2 * g], sc, -mA_new));
+      const float a1 = ex2_approx(fmaf(xa[2 * g + 1], sc, -mA_new));
+      const float b0 = ex2_approx(fmaf(xb[2 * g], sc, -mB_new));
+      const float b1 = ex2_approx(fmaf(xb[2 * g + 1], sc, -mB_new));
+      sumA += a0 + a1;
+      sumB += b0 + b1;
+      pa[g] = pack_bf16x2(a0, a1);
+      pb[g] = pack_bf16x2(b0, b1);
+    }
+    lA = lA * alphaA + sumA;
+    lB = lB * alphaB + sumB;
+    mA = mA_new;
+    mB = mB_new;
+
+    if (j > 0) {
+      mbar_wait(smem_u32(&ctl->o_done), (j - 1) & 1);  // PV(j-1) done: P and O are ours
+      tc_fence_after();
+      if (any) {
+#pragma unroll
+        for (int c0 = 0; c0 < D; c0 += 64) {
+          uint32_t o[32];
+          tmem_ld16x256_x8(tO + c0, o);
+          tmem_ld_wait();
+#pragma unroll
+          for (int g = 0; g < 8; ++g) {
+            o[4 * g] = __float_as_uint(__uint_as_float(o[4 * g]) * alphaA);
+            o[4 * g + 1] = __float_as_uint(__uint_as_float(o[4 * g + 1]) * alphaA);
+            o[4 * g + 2] = __float_as_uint(__uint_as_float(o[4 * g + 2]) * alphaB);
+            o[4 * g + 3] = __float_as_uint(__uint_as_float(o[4 * g + 3]) * alphaB);
+          }
+          tmem_st16x256_x8(tO + c0, o);
+        }
+        tmem_st_wait();
+      }
+    }
+    // P tile [64 rows x 64 keys] bf16, K-major, 128B swizzle: 16-byte chunk g of row r sits at
+    // chunk (g ^ (r & 7)); a quad's four 4-byte stores fill one chunk, the 8 rows of a store
+    // instruction hit 8 different chunks -> 32 distinct banks.
+#pragma unroll
+    for (int g = 0; g < 8; ++g) {
+      *reinterpret_cast<uint32_t*>(prowA + ((g ^ sw) << 4)) = pa[g];
+      *reinterpret_cast<uint32_t*>(prowB + ((g ^ sw) << 4)) = pb[g];
+    }
+    fence_proxy_async_smem();
+    tc_fence_before();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(smem_u32(&ctl->p_full));
+  }
+  // ---- epilogue: O / l -> bf16 -> global ---------------------------------------------------------
+  mbar_wait(smem_u32(&ctl->o_done), (n_it - 1) & 1);
+  tc_fence_after();
+  lA += __shfl_xor_sync(0xffffffffu, lA, 1);
+  lB += __shfl_xor_sync(0xffffffffu, lB, 1);
+  lA += __shfl_xor_sync(0xffffffffu, lA, 2);
+  lB += __shfl_xor_sync(0xffffffffu, lB, 2);
+  const float invA = 1.0f / lA, invB = 1.0f / lB;
+  const bool stA = qrA < p.N, stB = qrB < p.N;
+  uint16_t* obase = p.O + b * p.qsb + h * p.qsh + 2 * quad;
+  uint16_t* orowA = obase + static_cast<int64_t>(qrA) * p.qsn;
+  uint16_t* orowB = obase + static_cast<int64_t>(qrB) * p.qsn;
+#pragma unroll
+  for (int c0 = 0; c0 < D; c0 += 64) {
+    uint32_t o[32];
+    tmem_ld16x256_x8(tO + c0, o);
+    tmem_ld_wait();
+#pragma unroll
+    for (int g = 0; g < 8; ++g) {
+      const uint32_t va = pack_bf16x2(__uint_as_float(o[4 * g]) * invA, __uint_as_float(o[4 * g + 1]) * invA);
+      const uint32_t vb = pack_bf16x2(__uint_as_float(o[4 * g + 2]) * invB, __uint_as_float(o[4 * g + 3]) * invB);
+      if (stA) *reinterpret_cast<uint32_t*>(orowA + c0 + 8 * g) = va;
+      if (stB) *reinterpret_cast<uint32_t*>(orowB + c0 + 8 * g) = vb;
+    }
+  }
+  if (p.lse && quad == 0) {
+    float* lse = p.lse + (static_cast<int64_t>(b) * p.H + h) * p.N;
+    if (stA) lse[qrA] = (mA + log2f(lA)) * 0.6931471805599453f;
+    if (stB) lse[qrB] = (mB + log2f(lB)) * 0.6931471805599453f;
+  }
+  tc_fence_before();
+}
+
 template <int BM, int D, bool SPARSE>
 __global__ void __launch_bounds__(kThreads, Cfg<BM, D>::kOcc)
 attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
@@ -74,11 +337,17 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
   Ctl* ctl = reinterpret_cast<Ctl*>(kv_s + C::NS * C::KV_BYTES);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  // work item: heaviest (largest tile index) first
-  const int per_tile = p.B * p.H;
-  const int tq = p.NT - 1 - static_cast<int>(blockIdx.x) / per_tile;
-  const int rem = static_cast<int>(blockIdx.x) % per_tile;
-  const int b = rem / p.H, h = rem % p.H, g = h / p.G;
+  // work item order: (batch, KV head) outermost so that the CTAs in flight at any moment gather
+  // from ONE KV head's K/V (N*d*4 bytes: 67 MB at 128K, d=128 -- resident in the 126 MB L2) instead
+  // of all of them; inside a KV head the heaviest (largest tile index) tiles go first, and the G
+  // query heads of the group run side by side.
+  int wi = static_cast<int>(blockIdx.x);
+  const int hi = wi % p.G;
+  wi /= p.G;
+  const int tq = p.NT - 1 - wi % p.NT;
+  wi /= p.NT;
+  const int Hkv = p.H / p.G;
+  const int g = wi % Hkv, b = wi / Hkv, h = g * p.G + hi;
   const int q0 = tq * BM;  // first query row of this tile
 
   if ((smem_u32(smem) & 1023u) != 0) __trap();
@@ -201,111 +470,11 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
       }
     } else {
       // ---- softmax warps ---------------------------------------------------------------------
-      const bool active = (BM == 128) || (lane < 16);
-      const int r = (BM == 128) ? tid : (warp * 16 + (lane & 15));
-      const int qrow = q0 + r;
-      const uint32_t lane_base = static_cast<uint32_t>(warp * 32) << 16;
-      const uint32_t tS = tmem + lane_base, tO = tmem + lane_base + C::O_COL;
-      float m = -INFINITY, l = 0.f;
-      for (int j = 0; j < n_it; ++j) {
-        const int k0 = key_start(j);
-        mbar_wait(smem_u32(&ctl->s_full), j & 1);
-        tc_fence_after();
-        uint32_t sa[32], sb[32];
-        tmem_ld32(tS, sa);
-        tmem_ld32(tS + 32, sb);
-        tmem_ld_wait();
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&ctl->s_free));
-
-        float x[64];
-        const bool need_mask = (k0 + BN - 1 > q0);
-#pragma unroll
-        for (int c = 0; c < 32; ++c) {
-          x[c] = __uint_as_float(sa[c]) * p.scale_log2;
-          x[c + 32] = __uint_as_float(sb[c]) * p.scale_log2;
-        }
-        if (need_mask) {
-#pragma unroll
-          for (int c = 0; c < 64; ++c) x[c] = (k0 + c <= qrow) ? x[c] : -INFINITY;
-        }
-        float mx = x[0];
-#pragma unroll
-        for (int c = 1; c < 64; ++c) mx = fmaxf(mx, x[c]);
-        float m_new = fmaxf(m, mx);
-        // lazy rescale: keep the stale reference max unless some row of this warp grew by > 2^8
-        const bool grow = active && (m_new - m > 8.0f);
-        const bool any = __any_sync(0xffffffffu, grow);
-        if (!any) m_new = m;
-        const float alpha = ex2_approx(m - m_new);
-        float sum = 0.f;
-        uint32_t pk[32];
-#pragma unroll
-        for (int c = 0; c < 64; c += 2) {
-          const float e0 = ex2_approx(x[c] - m_new), e1 = ex2_approx(x[c + 1] - m_new);
-          sum += e0 + e1;
-          pk[c >> 1] = pack_bf16x2(e0, e1);
-        }
-        l = l * alpha + sum;
-        m = m_new;
-
-        if (j > 0) {
-          mbar_wait(smem_u32(&ctl->o_done), (j - 1) & 1);  // PV(j-1) done: P and O are ours
-          tc_fence_after();
-          if (any) {
-#pragma unroll
-            for (int c0 = 0; c0 < D; c0 += 32) {
-              uint32_t o[32];
-              tmem_ld32(tO + c0, o);
-              tmem_ld_wait();
-#pragma unroll
-              for (int c = 0; c < 32; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * alpha);
-              tmem_st32(tO + c0, o);
-            }
-            tmem_st_wait();
-          }
-        }
-        if (active) {
-          uint8_t* prow = p_s + r * 128;
-#pragma unroll
-          for (int c = 0; c < 8; ++c) {
-            uint4 v = make_uint4(pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
-            *reinterpret_cast<uint4*>(prow + ((c ^ (r & 7)) << 4)) = v;
-          }
-        }
-        fence_proxy_async_smem();
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&ctl->p_full));
+      if constexpr (BM == 64) {
+        softmax_m64<D, SPARSE>(p, ctl, p_s, tmem, n_it, q0, b, h, key_start);
+      } else {
+        softmax_m128<D, SPARSE>(p, ctl, p_s, tmem, n_it, q0, b, h, key_start);
       }
-      // ---- epilogue: O / l -> bf16 -> global ---------------------------------------------------
-      mbar_wait(smem_u32(&ctl->o_done), (n_it - 1) & 1);
-      tc_fence_after();
-      const float inv_l = 1.0f / l;
-      const bool store = active && (qrow < p.N);
-      uint16_t* orow = p.O + b * p.qsb + h * p.qsh + static_cast<int64_t>(qrow) * p.qsn;
-#pragma unroll
-      for (int c0 = 0; c0 < D; c0 += 32) {
-        uint32_t o[32];
-        tmem_ld32(tO + c0, o);
-        tmem_ld_wait();
-        if (store) {
-#pragma unroll
-          for (int c = 0; c < 32; c += 8) {
-            uint4 v;
-            v.x = pack_bf16x2(__uint_as_float(o[c]) * inv_l, __uint_as_float(o[c + 1]) * inv_l);
-            v.y = pack_bf16x2(__uint_as_float(o[c + 2]) * inv_l, __uint_as_float(o[c + 3]) * inv_l);
-            v.z = pack_bf16x2(__uint_as_float(o[c + 4]) * inv_l, __uint_as_float(o[c + 5]) * inv_l);
-            v.w = pack_bf16x2(__uint_as_float(o[c + 6]) * inv_l, __uint_as_float(o[c + 7]) * inv_l);
-            *reinterpret_cast<uint4*>(orow + c0 + c) = v;
-          }
-        }
-      }
-      if (store && p.lse)
-        p.lse[(static_cast<int64_t>(b) * p.H + h) * p.N + qrow] =
-            (m + log2f(l)) * 0.6931471805599453f;
-      tc_fence_before();
     }
   } else if (warp < 4) {
     // nothing attended (possible only with a caller-provided kv_idx): zeros, lse = -inf
