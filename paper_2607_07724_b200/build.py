@@ -8,6 +8,7 @@ repository snapshot.
 from __future__ import annotations
 
 import os
+import shlex
 import shutil
 import subprocess
 import sys
@@ -18,6 +19,7 @@ LIB = os.path.join(_HERE, "libbsa.so")
 SOURCES = ["api.cu", "pool.cu", "select.cu", "score_tc.cu", "attn.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
+NVCC_FLAGS += shlex.split(os.environ.get("BSA_NVCC_FLAGS", ""))   # developer knob, e.g. -DBSA_TC_OCC2=0
 
 
 def _nvcc() -> str:

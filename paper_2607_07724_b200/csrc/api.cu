@@ -83,6 +83,18 @@ static bsa_status check_device() {
   return BSA_OK;
 }
 
+int sm_count() {
+  static int cached[64] = {0};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 148;
+  if (cached[dev] == 0) {
+    int n = 0;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+    cached[dev] = n;
+  }
+  return cached[dev];
+}
+
 static bool policy_ok(int p) { return p >= BSA_POLICY_TOPK && p <= BSA_POLICY_ROUTER_QUEST; }
 static bool is_router(int p) { return p == BSA_POLICY_ROUTER || p == BSA_POLICY_ROUTER_QUEST; }
 

@@ -18,6 +18,7 @@ struct Dims {
 
 bsa_status fail(bsa_status code, const char* fmt, ...);
 bsa_status check_launch(const char* what);
+int sm_count();  // SMs of the current device (cached per device; 148 on B200)
 
 // meta plane offsets in bytes (see include/bsa.h); the three bf16 split planes of kmean
 // (hi, mid, lo; hi+mid+lo == kmean exactly) follow kmax and feed the tensor-core scoring.

@@ -29,12 +29,6 @@ __device__ __forceinline__ uint16_t f2bf_rn(float f) {
   return __bfloat16_as_ushort(__float2bfloat16_rn(f));
 }
 
-// Error-free fp32 addition (Knuth TwoSum): s + e == a + b exactly.
-__device__ __forceinline__ void two_sum(float a, float b, float& s, float& e) {
-  s = __fadd_rn(a, b);
-  const float bb = __fsub_rn(s, a);
-  e = __fadd_rn(__fsub_rn(a, __fsub_rn(s, bb)), __fsub_rn(b, bb));
-}
 __device__ __forceinline__ uint32_t bf2_min(uint32_t a, uint32_t b) {
   uint32_t r;
   asm("min.bf16x2 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b));
@@ -48,63 +42,85 @@ __device__ __forceinline__ uint32_t bf2_max(uint32_t a, uint32_t b) {
 
 constexpr int kPasses = 8;  // key rows per thread: 8 x 16 B = 128 B in flight per thread
 
-// One CTA of BN*D/64 threads per (batch, KV head, block).  Thread (r0, c8) owns 8 adjacent
-// columns of rows r0, r0 + RPP, ..., all 8 loads issued before the first use.  The column sum is
-// exact: a TwoSum chain in fp32 carries the running sum, and the (almost always zero) rounding
-// errors of the chain are detected with one OR; only a thread that saw a non-zero error re-adds
-// its 8 rows in fp64.  Partial sums are then combined across threads in fp64 (exact for bf16
-// inputs), so the mean is the correctly rounded fp32 mean whatever the order -- without paying an
-// fp32->fp64 conversion (XU pipe, quarter rate) per element.
+// CTAs of BN*D/64 threads; thread (r0, c8) owns 8 adjacent columns of rows r0, r0 + RPP, ... of a
+// block (8 x 16 B loads).  The per-thread column sums run in fp32 with a two-adds-per-element
+// exactness test (see process_block); only a thread whose test fails re-adds its 8 rows in fp64.
+// Partial sums are combined across threads in fp64 (exact for bf16 inputs), so the mean is the
+// correctly rounded fp32 mean whatever the order -- without an fp32->fp64 conversion (XU pipe,
+// quarter rate) per element.  min / max stay packed bf16x2 until the last step.
 template <int D, int BN>
-__global__ void __launch_bounds__(BN* D / 64, 768 / (BN * D / 64)) pool_kernel(const uint16_t* __restrict__ K, int64_t ksb,
-                                                         int64_t ksh, int64_t ksn, int NB, int Hkv,
-                                                         int kinds, float* __restrict__ kmean,
-                                                         uint16_t* __restrict__ kmin,
-                                                         uint16_t* __restrict__ kmax,
-                                                         uint16_t* __restrict__ ksplit,
-                                                         size_t plane_elems) {
+struct PoolArgs {
+  const uint16_t* K;
+  int64_t ksb, ksh, ksn;
+  int NB, Hkv, B, kinds;
+  float* kmean;
+  uint16_t *kmin, *kmax, *ksplit;
+  size_t plane_elems;
+};
+
+// work item w -> (batch b, KV head g, block blk); rows r0 + p*RPP of that block, 8 columns at c8*8
+template <int D, int BN>
+__device__ __forceinline__ void load_block(const PoolArgs<D, BN>& a, int w, uint4 (&v)[kPasses]) {
+  constexpr int kThreads = BN * D / 64, TPR = D / 8, RPP = kThreads / TPR;
+  const int blk = w % a.NB, g = (w / a.NB) % a.Hkv, b = w / (a.NB * a.Hkv);
+  const int c8 = threadIdx.x % TPR, r0 = threadIdx.x / TPR;
+  const uint16_t* base = a.K + b * a.ksb + g * a.ksh + static_cast<int64_t>(blk) * BN * a.ksn + c8 * 8;
+#pragma unroll
+  for (int p = 0; p < kPasses; ++p)
+    v[p] = ld_stream(reinterpret_cast<const uint4*>(base + static_cast<int64_t>(r0 + p * RPP) * a.ksn));
+}
+
+template <int D, int BN>
+__device__ __forceinline__ void process_block(const PoolArgs<D, BN>& a, int w, const uint4 (&v)[kPasses]) {
   constexpr int kThreads = BN * D / 64;
   constexpr int TPR = D / 8;            // threads per key row (8 bf16 = 16 B each)
   constexpr int RPP = kThreads / TPR;   // rows per pass
   static_assert(RPP * kPasses == BN, "thread count must give exactly kPasses rows per thread");
-  const int blk = blockIdx.x, g = blockIdx.y, b = blockIdx.z;
+  const int blk = w % a.NB, g = (w / a.NB) % a.Hkv, b = w / (a.NB * a.Hkv);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int c8 = tid % TPR, r0 = tid / TPR;
+  const int c8 = tid % TPR;
+  const int NB = a.NB, Hkv = a.Hkv, kinds = a.kinds;
+  float* __restrict__ kmean = a.kmean;
+  uint16_t* __restrict__ kmin = a.kmin;
+  uint16_t* __restrict__ kmax = a.kmax;
+  uint16_t* __restrict__ ksplit = a.ksplit;
+  const size_t plane_elems = a.plane_elems;
 
-  const uint16_t* base = K + b * ksb + g * ksh + static_cast<int64_t>(blk) * BN * ksn + c8 * 8;
-  uint4 v[kPasses];
-#pragma unroll
-  for (int p = 0; p < kPasses; ++p)
-    v[p] = ld_stream(reinterpret_cast<const uint4*>(base + static_cast<int64_t>(r0 + p * RPP) * ksn));
-
-  float hi[8];
+  // Exactness test that costs two adds per element: the same chain is run once rounding every add
+  // up and once rounding it down.  ru >= exact >= rd holds inductively, and the first inexact add
+  // opens a gap that later adds can only keep (RU(a' + y) >= a' + y > a + y >= RD(a + y) for
+  // a' > a), so ru == rd at the end  <=>  every add was exact  <=>  ru is the exact column sum.
+  float ru[8], rd[8];
   uint32_t mn2[4], mx2[4];
   {
     const uint32_t w[4] = {v[0].x, v[0].y, v[0].z, v[0].w};
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-      hi[2 * i] = bf_lo(w[i]);
-      hi[2 * i + 1] = bf_hi(w[i]);
+      ru[2 * i] = rd[2 * i] = bf_lo(w[i]);
+      ru[2 * i + 1] = rd[2 * i + 1] = bf_hi(w[i]);
       mn2[i] = w[i];
       mx2[i] = w[i];
     }
   }
-  uint32_t err_bits = 0;
 #pragma unroll
   for (int p = 1; p < kPasses; ++p) {
     const uint32_t w[4] = {v[p].x, v[p].y, v[p].z, v[p].w};
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-      float e0, e1;
-      two_sum(hi[2 * i], bf_lo(w[i]), hi[2 * i], e0);
-      two_sum(hi[2 * i + 1], bf_hi(w[i]), hi[2 * i + 1], e1);
-      err_bits |= __float_as_uint(e0) | __float_as_uint(e1);
+      const float lo = bf_lo(w[i]), hv = bf_hi(w[i]);
+      ru[2 * i] = __fadd_ru(ru[2 * i], lo);
+      rd[2 * i] = __fadd_rd(rd[2 * i], lo);
+      ru[2 * i + 1] = __fadd_ru(ru[2 * i + 1], hv);
+      rd[2 * i + 1] = __fadd_rd(rd[2 * i + 1], hv);
       mn2[i] = bf2_min(mn2[i], w[i]);
       mx2[i] = bf2_max(mx2[i], w[i]);
     }
   }
+  bool exact = true;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) exact = exact && (ru[i] == rd[i]);
   double sum[8];
-  if ((err_bits << 1) != 0) {  // some fp32 add was inexact (an error of -0 does not count): redo in fp64
+  if (!exact) {  // some fp32 add was inexact: redo this thread's rows in fp64
 #pragma unroll
     for (int i = 0; i < 8; ++i) sum[i] = 0.0;
 #pragma unroll
@@ -118,40 +134,31 @@ __global__ void __launch_bounds__(BN* D / 64, 768 / (BN * D / 64)) pool_kernel(c
     }
   } else {
 #pragma unroll
-    for (int i = 0; i < 8; ++i) sum[i] = static_cast<double>(hi[i]);
-  }
-  float mn[8], mx[8];
-#pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    mn[2 * i] = bf_lo(mn2[i]);
-    mn[2 * i + 1] = bf_hi(mn2[i]);
-    mx[2 * i] = bf_lo(mx2[i]);
-    mx[2 * i + 1] = bf_hi(mx2[i]);
+    for (int i = 0; i < 8; ++i) sum[i] = static_cast<double>(ru[i]);
   }
   // rows that live in the same warp (lanes that differ by a multiple of TPR)
 #pragma unroll
   for (int off = 16; off >= TPR; off >>= 1) {
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-      sum[i] += __shfl_xor_sync(0xffffffffu, sum[i], off);
-      mn[i] = fminf(mn[i], __shfl_xor_sync(0xffffffffu, mn[i], off));
-      mx[i] = fmaxf(mx[i], __shfl_xor_sync(0xffffffffu, mx[i], off));
+    for (int i = 0; i < 8; ++i) sum[i] += __shfl_xor_sync(0xffffffffu, sum[i], off);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      mn2[i] = bf2_min(mn2[i], __shfl_xor_sync(0xffffffffu, mn2[i], off));
+      mx2[i] = bf2_max(mx2[i], __shfl_xor_sync(0xffffffffu, mx2[i], off));
     }
   }
   constexpr int NW = kThreads / 32;
   constexpr int CW = (TPR <= 32) ? 1 : TPR / 32;   // warps that cover one key row
   constexpr int NR = NW / CW;                       // partial results per column
   __shared__ double s_sum[NR][D];
-  __shared__ uint16_t s_mn[NR][D], s_mx[NR][D];
+  __shared__ uint32_t s_mn[NR][D / 2], s_mx[NR][D / 2];  // bf16x2
   constexpr int LPW = (TPR < 32) ? TPR : 32;  // distinct column groups per warp
   if (lane < LPW) {
     const int col = c8 * 8;
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-      s_sum[warp / CW][col + i] = sum[i];
-      s_mn[warp / CW][col + i] = f2bf_exact(mn[i]);
-      s_mx[warp / CW][col + i] = f2bf_exact(mx[i]);
-    }
+    for (int i = 0; i < 8; ++i) s_sum[warp / CW][col + i] = sum[i];
+    *reinterpret_cast<uint4*>(&s_mn[warp / CW][col / 2]) = make_uint4(mn2[0], mn2[1], mn2[2], mn2[3]);
+    *reinterpret_cast<uint4*>(&s_mx[warp / CW][col / 2]) = make_uint4(mx2[0], mx2[1], mx2[2], mx2[3]);
   }
   __syncthreads();
   for (int c = tid; c < D; c += kThreads) {
@@ -160,8 +167,9 @@ __global__ void __launch_bounds__(BN* D / 64, 768 / (BN * D / 64)) pool_kernel(c
 #pragma unroll
     for (int w = 0; w < NR; ++w) {
       s += s_sum[w][c];
-      lo = fminf(lo, __uint_as_float(static_cast<uint32_t>(s_mn[w][c]) << 16));
-      hv = fmaxf(hv, __uint_as_float(static_cast<uint32_t>(s_mx[w][c]) << 16));
+      const uint32_t wn = s_mn[w][c >> 1], wx = s_mx[w][c >> 1];
+      lo = fminf(lo, (c & 1) ? bf_hi(wn) : bf_lo(wn));
+      hv = fmaxf(hv, (c & 1) ? bf_hi(wx) : bf_lo(wx));
     }
     const size_t o = ((static_cast<size_t>(b) * Hkv + g) * NB + blk) * D + c;
     if (kinds & BSA_META_MEAN) {
@@ -184,14 +192,29 @@ __global__ void __launch_bounds__(BN* D / 64, 768 / (BN * D / 64)) pool_kernel(c
 }
 
 template <int D, int BN>
+__global__ void __launch_bounds__(BN* D / 64, 768 / (BN * D / 64)) pool_kernel(const PoolArgs<D, BN> a) {
+  uint4 v[kPasses];
+  load_block<D, BN>(a, static_cast<int>(blockIdx.x), v);
+  process_block<D, BN>(a, static_cast<int>(blockIdx.x), v);
+}
+
+template <int D, int BN>
 void launch(const Dims& S, const void* K, int kinds, char* meta, const MetaLayout& L,
             cudaStream_t stream) {
-  dim3 grid(S.NB, S.Hkv, S.B);
-  pool_kernel<D, BN><<<grid, BN * D / 64, 0, stream>>>(
-      static_cast<const uint16_t*>(K), S.ksb, S.ksh, S.ksn, S.NB, S.Hkv, kinds,
-      reinterpret_cast<float*>(meta + L.off_mean), reinterpret_cast<uint16_t*>(meta + L.off_min),
-      reinterpret_cast<uint16_t*>(meta + L.off_max), reinterpret_cast<uint16_t*>(meta + L.off_split),
-      L.elems);
+  PoolArgs<D, BN> a;
+  a.K = static_cast<const uint16_t*>(K);
+  a.ksb = S.ksb; a.ksh = S.ksh; a.ksn = S.ksn;
+  a.NB = S.NB; a.Hkv = S.Hkv; a.B = S.B; a.kinds = kinds;
+  a.kmean = reinterpret_cast<float*>(meta + L.off_mean);
+  a.kmin = reinterpret_cast<uint16_t*>(meta + L.off_min);
+  a.kmax = reinterpret_cast<uint16_t*>(meta + L.off_max);
+  a.ksplit = reinterpret_cast<uint16_t*>(meta + L.off_split);
+  a.plane_elems = L.elems;
+  constexpr int kThreads = BN * D / 64;
+  const int total = S.NB * S.Hkv * S.B;
+  // one block per CTA: with ~6 CTAs resident per SM their load and reduce phases interleave; a
+  // persistent register-double-buffered variant measured 25 % slower (fewer warps to hide the adds)
+  pool_kernel<D, BN><<<total, kThreads, 0, stream>>>(a);
 }
 
 }  // namespace

@@ -1,7 +1,7 @@
 // score_tc.cu -- tensor-core block scoring fused with tile-max, top-(2k) and sigma
 // (Eq.1-4; A.2-A.6 L296-324; readings G1, G4-G8 in DESIGN.md).
 //
-// One CTA per (tile t, KV head g, head set) where a head set is up to NH query heads of the GQA
+// Work item = (tile t, KV head g, head set) where a head set is up to NH query heads of the GQA
 // group.  The product is computed TRANSPOSED so that the tile max (Eq.3) is a per-thread loop:
 //     S^T[block, (head, row)] = Pooled[block, :] . Qplanes[(head, row), :]
 //   A (M = 128 pooled blocks, K-major)  streamed by TMA from the meta planes through a ring,
@@ -11,8 +11,18 @@
 //   q- = min(q,0); all four operands are bf16-exact, K dimension 2d.
 // K-mean (Eq.1): kmean (fp32) = hi + mid + lo exactly (three bf16 planes written by the pooling
 //   kernel), K dimension 3d against the same Q chunk; products are exact, accumulation is fp32.
-// Warps 0-3: Q+/Q- conversion, epilogue (column max per head -> shared-memory score rows), then one
-//   warp per head runs warp_select (select_common.cuh).   Warp 4: TMA producer.   Warp 5: MMA issue.
+//
+// The kernel is PERSISTENT (one CTA per SM, items strided over the grid, heaviest tiles first) and
+// software-pipelined across items, because a one-item CTA spends ~10 us in phases that leave the
+// tensor pipe idle (Q load 1.7k clk, q+/q- conversion 1.9k, ring warm-up, selection 6-8k) against
+// 1-2 us of MMAs at 32K.  Roles (10 warps):
+//   W0-3  q+/q- conversion of the item's Q tile, then the per-chunk epilogue: TMEM -> column max
+//         per head -> order-preserving key -> score row in shared memory
+//   W4    TMA producer: Q tile of the next item as soon as the MMAs of the current one are done,
+//         pooled planes through the ring, continuously across items
+//   W5    tcgen05.mma issue, accumulators ping-pong across chunks and items
+//   W6-9  one warp per head: warp_select (select_common.cuh) of item i while W0-5 already work on
+//         item i+1; the score rows are released as soon as the warp holds its keys in registers
 #include <cuda_bf16.h>
 
 #include "bsa_internal.h"
@@ -24,10 +34,11 @@ namespace bsa {
 
 namespace {
 
-constexpr int kTcThreads = 192;
+constexpr int kTcThreads = 320;
 constexpr int kABlocks = 128;                 // pooled blocks per MMA (UMMA M)
 constexpr int kAStageBytes = kABlocks * 128;  // one [128 blocks x 64 elem] swizzled tile
 constexpr int kMaxStages = 6;
+constexpr int kSelWarp0 = 6;                  // first selection warp
 
 template <int D, int BN, bool QUEST>
 struct TcCfg {
@@ -35,7 +46,7 @@ struct TcCfg {
   static constexpr int PLANES_A = QUEST ? 2 : 3;          // kmax | kmin   or   hi | mid | lo
   static constexpr int DC = D / 64;                        // 64-element K chunks per plane
   static constexpr int HEAD_B_BYTES = BN * D * 2 * PLANES_B;
-  static constexpr int NH_N = 256 / BN;                    // UMMA N <= 256
+  static constexpr int NH_N = 256 / BN;                    // UMMA N <= 256; also <= 4 selection warps
   static constexpr int NH_S = (128 * 1024) / HEAD_B_BYTES; // B planes <= 128 KB
   static constexpr int NH = NH_N < NH_S ? NH_N : NH_S;
   static constexpr int NROWS = NH * BN;                    // rows of one B chunk tile
@@ -44,27 +55,45 @@ struct TcCfg {
   static constexpr int KCHUNKS = PLANES_A * DC;            // A chunks per block chunk
   static constexpr uint32_t TMEM_COLS = (2 * NROWS <= 32) ? 32 : (2 * NROWS <= 64) ? 64
                                         : (2 * NROWS <= 128) ? 128 : (2 * NROWS <= 256) ? 256 : 512;
-  static_assert(NH >= 1, "B planes of one head do not fit");
+  static_assert(NH >= 1 && NH <= 4, "one selection warp per head, four of them");
 };
 
 struct TcParams {
   int32_t* kv_idx;
   int32_t* kv_count;
   float* sigma;
-  int B, H, Hkv, G, NB, k, W, router, sets, stages, nbpad;
+  int B, H, Hkv, G, NB, k, W, router, sets, stages, nbpad, n_items;
   float inv_sqrt_d;
 };
 
 struct alignas(8) TcCtl {
-  uint64_t q_full, b_ready;
+  uint64_t q_full, b_ready, b_free, sc_full, sc_free;
   uint64_t a_full[kMaxStages], a_empty[kMaxStages];
   uint64_t acc_full[2], acc_empty[2];
   uint32_t tmem_base;
   uint32_t s3[4 * 4];   // per-warp scratch of warp_select
 };
 
-__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
-  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+struct Item {
+  int t, b, g, set, h0, nh, n_chunks;
+};
+
+// item w -> (tile, batch, KV head, head set); heaviest (largest t) tiles first
+template <int NH>
+__device__ __forceinline__ Item decode_item(const TcParams& p, int w) {
+  Item it;
+  const int per_tile = p.B * p.Hkv * p.sets;
+  it.t = p.NB - 1 - w / per_tile;
+  int rem = w % per_tile;
+  it.b = rem / (p.Hkv * p.sets);
+  rem %= p.Hkv * p.sets;
+  it.g = rem / p.sets;
+  it.set = rem % p.sets;
+  it.h0 = it.g * p.G + it.set * NH;
+  const int left = p.G - it.set * NH;
+  it.nh = left < NH ? left : NH;
+  it.n_chunks = (it.t + 1 + kABlocks - 1) / kABlocks;
+  return it;
 }
 
 template <int D, int BN, bool QUEST>
@@ -80,22 +109,16 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   TcCtl* ctl = reinterpret_cast<TcCtl*>(cand + C::NH * kMaxCand);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  // unit: heaviest tiles first
-  const int per_tile = p.B * p.Hkv * p.sets;
-  const int t = p.NB - 1 - static_cast<int>(blockIdx.x) / per_tile;
-  int rem = static_cast<int>(blockIdx.x) % per_tile;
-  const int b = rem / (p.Hkv * p.sets);
-  rem %= p.Hkv * p.sets;
-  const int g = rem / p.sets, set = rem % p.sets;
-  const int h0 = g * p.G + set * C::NH;
-  const int nh = (p.G - set * C::NH) < C::NH ? (p.G - set * C::NH) : C::NH;   // heads in this set
-  const int n_chunks = (t + 1 + kABlocks - 1) / kABlocks;
+  const int w0 = static_cast<int>(blockIdx.x), wstep = static_cast<int>(gridDim.x);
 
   if ((smem_u32(smem) & 1023u) != 0) __trap();
 
   if (warp == 5 && lane == 0) {
     mbar_init(smem_u32(&ctl->q_full), 1);
     mbar_init(smem_u32(&ctl->b_ready), 4);
+    mbar_init(smem_u32(&ctl->b_free), 1);
+    mbar_init(smem_u32(&ctl->sc_full), 4);
+    mbar_init(smem_u32(&ctl->sc_free), 4);
     for (int s = 0; s < p.stages; ++s) {
       mbar_init(smem_u32(&ctl->a_full[s]), 1);
       mbar_init(smem_u32(&ctl->a_empty[s]), 1);
@@ -122,111 +145,144 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   if (warp == 4) {
     // ---- TMA producer ------------------------------------------------------------------------
     if (lane == 0) {
-      mbar_arrive_expect_tx(smem_u32(&ctl->q_full), C::DC * C::B_CHUNK_BYTES);
-      for (int c64 = 0; c64 < C::DC; ++c64)
-        tma_load_5d(smem_u32(b_s + c64 * C::B_CHUNK_BYTES), &tmQ, smem_u32(&ctl->q_full), 0, t * BN,
-                    c64, h0, b);
-      int it = 0;
-      for (int c = 0; c < n_chunks; ++c) {
-        for (int kc = 0; kc < C::KCHUNKS; ++kc, ++it) {
-          const int s = it % p.stages;
-          const int pa = kc / C::DC, c64 = kc % C::DC;
-          const int mem_plane = QUEST ? (1 - pa) : pa;   // memory order: [kmin, kmax] / [hi, mid, lo]
-          mbar_wait(smem_u32(&ctl->a_empty[s]), ((it / p.stages) & 1) ^ 1);
-          mbar_arrive_expect_tx(smem_u32(&ctl->a_full[s]), kAStageBytes);
-          tma_load_5d(smem_u32(a_s + s * kAStageBytes), &tmA, smem_u32(&ctl->a_full[s]), c64 * 64,
-                      c * kABlocks, g, b, mem_plane);
+      int li = 0, ring = 0;
+      for (int w = w0; w < p.n_items; w += wstep, ++li) {
+        const Item im = decode_item<C::NH>(p, w);
+        if (li > 0) mbar_wait(smem_u32(&ctl->b_free), (li - 1) & 1);   // MMAs of the previous item done
+        mbar_arrive_expect_tx(smem_u32(&ctl->q_full), C::DC * C::B_CHUNK_BYTES);
+        for (int c64 = 0; c64 < C::DC; ++c64)
+          tma_load_5d(smem_u32(b_s + c64 * C::B_CHUNK_BYTES), &tmQ, smem_u32(&ctl->q_full), 0,
+                      im.t * BN, c64, im.h0, im.b);
+        if (w + wstep < p.n_items) {   // warm the L2 with the Q tile of this CTA's next item
+          const Item nx = decode_item<C::NH>(p, w + wstep);
+          for (int c64 = 0; c64 < C::DC; ++c64)
+            tma_prefetch_5d(&tmQ, 0, nx.t * BN, c64, nx.h0, nx.b);
+        }
+        for (int c = 0; c < im.n_chunks; ++c) {
+          for (int kc = 0; kc < C::KCHUNKS; ++kc, ++ring) {
+            const int s = ring % p.stages;
+            const int pa = kc / C::DC, c64 = kc % C::DC;
+            const int mem_plane = QUEST ? (1 - pa) : pa;   // memory order: [kmin, kmax] / [hi, mid, lo]
+            mbar_wait(smem_u32(&ctl->a_empty[s]), ((ring / p.stages) & 1) ^ 1);
+            mbar_arrive_expect_tx(smem_u32(&ctl->a_full[s]), kAStageBytes);
+            tma_load_5d(smem_u32(a_s + s * kAStageBytes), &tmA, smem_u32(&ctl->a_full[s]), c64 * 64,
+                        c * kABlocks, im.g, im.b, mem_plane);
+          }
         }
       }
     }
   } else if (warp == 5) {
     // ---- MMA issuer --------------------------------------------------------------------------
     if (lane == 0) {
-      const uint32_t idesc = umma_idesc_bf16(kABlocks, nh * BN, 0, 0);
       const uint32_t b_a = smem_u32(b_s), a_a = smem_u32(a_s);
-      mbar_wait(smem_u32(&ctl->b_ready), 0);
-      tc_fence_after();
-      int it = 0;
-      for (int c = 0; c < n_chunks; ++c) {
-        const int buf = c & 1;
-        if (c >= 2) {
-          mbar_wait(smem_u32(&ctl->acc_empty[buf]), ((c >> 1) & 1) ^ 1);
-          tc_fence_after();
-        }
-        const uint32_t tD = tmem + buf * C::NROWS;
-        for (int kc = 0; kc < C::KCHUNKS; ++kc, ++it) {
-          const int s = it % p.stages;
-          const int bchunk = QUEST ? kc : (kc % C::DC);
-          mbar_wait(smem_u32(&ctl->a_full[s]), (it / p.stages) & 1);
-          tc_fence_after();
-#pragma unroll
-          for (int ks = 0; ks < 4; ++ks) {
-            const uint64_t ad = umma_smem_desc(a_a + s * kAStageBytes + ks * 32, 16, 1024);
-            const uint64_t bd = umma_smem_desc(b_a + bchunk * C::B_CHUNK_BYTES + ks * 32, 16, 1024);
-            umma_ss(tD, ad, bd, idesc, (kc > 0) || (ks > 0));
+      int li = 0, ring = 0, cg = 0;
+      for (int w = w0; w < p.n_items; w += wstep, ++li) {
+        const Item im = decode_item<C::NH>(p, w);
+        const uint32_t idesc = umma_idesc_bf16(kABlocks, im.nh * BN, 0, 0);
+        mbar_wait(smem_u32(&ctl->b_ready), li & 1);
+        tc_fence_after();
+        for (int c = 0; c < im.n_chunks; ++c, ++cg) {
+          const int buf = cg & 1;
+          if (cg >= 2) {
+            mbar_wait(smem_u32(&ctl->acc_empty[buf]), ((cg >> 1) & 1) ^ 1);
+            tc_fence_after();
           }
-          tc_commit(smem_u32(&ctl->a_empty[s]));
-        }
-        tc_commit(smem_u32(&ctl->acc_full[buf]));
-      }
-    }
-  } else {
-    // ---- conversion, epilogue, selection (warps 0-3) -----------------------------------------
-    mbar_wait(smem_u32(&ctl->q_full), 0);
-    if (QUEST) {
-      // q+ = max(q, 0) in place, q- = min(q, 0) into plane 1 (element-wise, swizzle preserved)
-      constexpr int PLANE = C::DC * C::B_CHUNK_BYTES;
-      for (int i = tid; i < PLANE / 16; i += 128) {
-        uint4 v = *reinterpret_cast<uint4*>(b_s + i * 16);
-        uint32_t w[4] = {v.x, v.y, v.z, v.w}, pos[4], neg[4];
+          const uint32_t tD = tmem + buf * C::NROWS;
+          for (int kc = 0; kc < C::KCHUNKS; ++kc, ++ring) {
+            const int s = ring % p.stages;
+            const int bchunk = QUEST ? kc : (kc % C::DC);
+            mbar_wait(smem_u32(&ctl->a_full[s]), (ring / p.stages) & 1);
+            tc_fence_after();
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const uint32_t nm = ((w[j] & 0x80008000u) >> 15) * 0xFFFFu;  // 0xFFFF per negative half
-          neg[j] = w[j] & nm;
-          pos[j] = w[j] & ~nm;
+            for (int ks = 0; ks < 4; ++ks) {
+              const uint64_t ad = umma_smem_desc(a_a + s * kAStageBytes + ks * 32, 16, 1024);
+              const uint64_t bd = umma_smem_desc(b_a + bchunk * C::B_CHUNK_BYTES + ks * 32, 16, 1024);
+              umma_ss(tD, ad, bd, idesc, (kc > 0) || (ks > 0));
+            }
+            tc_commit(smem_u32(&ctl->a_empty[s]));
+          }
+          tc_commit(smem_u32(&ctl->acc_full[buf]));
         }
-        *reinterpret_cast<uint4*>(b_s + i * 16) = make_uint4(pos[0], pos[1], pos[2], pos[3]);
-        *reinterpret_cast<uint4*>(b_s + PLANE + i * 16) = make_uint4(neg[0], neg[1], neg[2], neg[3]);
+        tc_commit(smem_u32(&ctl->b_free));   // every MMA that reads this item's B planes has completed
       }
-      fence_proxy_async_smem();
     }
-    __syncwarp();
-    if (lane == 0) mbar_arrive(smem_u32(&ctl->b_ready));
-
+  } else if (warp < 4) {
+    // ---- conversion + epilogue (warps 0-3) ---------------------------------------------------
     const uint32_t lane_base = static_cast<uint32_t>(warp * 32) << 16;
-    for (int c = 0; c < n_chunks; ++c) {
-      const int buf = c & 1;
-      mbar_wait(smem_u32(&ctl->acc_full[buf]), (c >> 1) & 1);
-      tc_fence_after();
-      const int blk = c * kABlocks + warp * 32 + lane;
-      const uint32_t tD = tmem + lane_base + buf * C::NROWS;
-      for (int j = 0; j < nh; ++j) {
-        float mx = -INFINITY;
+    int li = 0, cg = 0;
+    for (int w = w0; w < p.n_items; w += wstep, ++li) {
+      const Item im = decode_item<C::NH>(p, w);
+      mbar_wait(smem_u32(&ctl->q_full), li & 1);
+      if (QUEST) {
+        // q+ = max(q, 0) in place, q- = min(q, 0) into plane 1 (element-wise, swizzle preserved)
+        constexpr int PLANE = C::DC * C::B_CHUNK_BYTES;
+#pragma unroll 4
+        for (int i = tid; i < PLANE / 16; i += 128) {
+          uint4 v = *reinterpret_cast<uint4*>(b_s + i * 16);
+          uint32_t wv[4] = {v.x, v.y, v.z, v.w}, pos[4], neg[4];
 #pragma unroll
-        for (int c0 = 0; c0 < BN; c0 += 64) {
-          uint32_t ra[32], rb[32];
-          tmem_ld32(tD + j * BN + c0, ra);
-          tmem_ld32(tD + j * BN + c0 + 32, rb);
-          tmem_ld_wait();
-#pragma unroll
-          for (int i = 0; i < 32; ++i)
-            mx = fmaxf(mx, fmaxf(__uint_as_float(ra[i]), __uint_as_float(rb[i])));
+          for (int j = 0; j < 4; ++j) {
+            const uint32_t nm = ((wv[j] & 0x80008000u) >> 15) * 0xFFFFu;  // 0xFFFF per negative half
+            neg[j] = wv[j] & nm;
+            pos[j] = wv[j] & ~nm;
+          }
+          *reinterpret_cast<uint4*>(b_s + i * 16) = make_uint4(pos[0], pos[1], pos[2], pos[3]);
+          *reinterpret_cast<uint4*>(b_s + PLANE + i * 16) = make_uint4(neg[0], neg[1], neg[2], neg[3]);
         }
-        if (blk <= t) sc[j * p.nbpad + blk] = okey(QUEST ? mx : mx * p.inv_sqrt_d);   // Eq.3 (G8)
+        fence_proxy_async_smem();
       }
-      tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(smem_u32(&ctl->acc_empty[buf]));
+      if (lane == 0) mbar_arrive(smem_u32(&ctl->b_ready));
+
+      // the selection warps must hold the previous item's keys in registers before sc is rewritten
+      if (li > 0) mbar_wait(smem_u32(&ctl->sc_free), (li - 1) & 1);
+      for (int c = 0; c < im.n_chunks; ++c, ++cg) {
+        const int buf = cg & 1;
+        mbar_wait(smem_u32(&ctl->acc_full[buf]), (cg >> 1) & 1);
+        tc_fence_after();
+        const int blk = c * kABlocks + warp * 32 + lane;
+        const uint32_t tD = tmem + lane_base + buf * C::NROWS;
+        for (int j = 0; j < im.nh; ++j) {
+          float mx = -INFINITY;
+#pragma unroll
+          for (int c0 = 0; c0 < BN; c0 += 64) {
+            uint32_t ra[32], rb[32];
+            tmem_ld32(tD + j * BN + c0, ra);
+            tmem_ld32(tD + j * BN + c0 + 32, rb);
+            tmem_ld_wait();
+#pragma unroll
+            for (int i = 0; i < 32; ++i)
+              mx = fmax3(mx, __uint_as_float(ra[i]), __uint_as_float(rb[i]));
+          }
+          if (blk <= im.t) sc[j * p.nbpad + blk] = okey(QUEST ? mx : mx * p.inv_sqrt_d);   // Eq.3 (G8)
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&ctl->acc_empty[buf]));
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(smem_u32(&ctl->sc_full));   // release: the score rows are complete
     }
-    named_bar_sync(1, 128);
-    if (warp < nh) {
-      const int h = h0 + warp;
-      const int64_t row = (static_cast<int64_t>(b) * p.H + h) * p.NB + t;
-      const float sig = warp_select(sc + warp * p.nbpad, t, p.k, p.NB, p.W, p.kv_idx + row * p.W,
-                                    cand + warp * kMaxCand, ctl->s3 + warp * 4, lane);
-      if (lane == 0) {
-        p.sigma[row] = sig;
-        if (!p.router) p.kv_count[row] = (p.k < t + 1) ? p.k : t + 1;
+  } else if (warp >= kSelWarp0) {
+    // ---- selection (warps 6-9, one per head) --------------------------------------------------
+    const int sw = warp - kSelWarp0;
+    int li = 0;
+    for (int w = w0; w < p.n_items; w += wstep, ++li) {
+      const Item im = decode_item<C::NH>(p, w);
+      mbar_wait(smem_u32(&ctl->sc_full), li & 1);
+      const uint32_t rel = smem_u32(&ctl->sc_free);
+      if (sw < im.nh && sw < C::NH) {
+        const int h = im.h0 + sw;
+        const int64_t row = (static_cast<int64_t>(im.b) * p.H + h) * p.NB + im.t;
+        const float sig = warp_select(sc + sw * p.nbpad, im.t, p.k, p.NB, p.W, p.kv_idx + row * p.W,
+                                      cand + sw * kMaxCand, ctl->s3 + sw * 4, lane, rel);
+        if (lane == 0) {
+          p.sigma[row] = sig;
+          if (!p.router) p.kv_count[row] = (p.k < im.t + 1) ? p.k : im.t + 1;
+        }
+        __syncwarp();   // cand / s3 of this warp are reused by the next item
+      } else {
+        release_keys(rel, lane);
       }
     }
   }
@@ -247,6 +303,9 @@ bsa_status run_score_tc(const Dims& S, const void* Q, const char* meta, const Me
   p.sets = (S.G + C::NH - 1) / C::NH;
   p.nbpad = (S.NB + 3) & ~3;
   p.inv_sqrt_d = static_cast<float>(1.0 / sqrt(static_cast<double>(S.d)));
+  const long long n_items = static_cast<long long>(S.NB) * S.B * S.Hkv * p.sets;
+  if (n_items > 0x7fffffffLL) return fail(BSA_ERR_UNSUPPORTED, "select: too many work items");
+  p.n_items = static_cast<int>(n_items);
   const size_t fixed = static_cast<size_t>(C::B_BYTES) + static_cast<size_t>(C::NH) * p.nbpad * 4 +
                        static_cast<size_t>(C::NH) * kMaxCand * 8 + sizeof(TcCtl);
   const size_t budget = 227 * 1024;
@@ -274,9 +333,9 @@ bsa_status run_score_tc(const Dims& S, const void* Q, const char* meta, const Me
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        static_cast<int>(smem));
   if (e != cudaSuccess) return fail(BSA_ERR_CUDA, "select: smem attribute: %s", cudaGetErrorString(e));
-  const long long grid = static_cast<long long>(S.NB) * S.B * S.Hkv * p.sets;
-  if (grid > 0x7fffffffLL) return fail(BSA_ERR_UNSUPPORTED, "select: grid too large");
-  kern<<<static_cast<unsigned>(grid), kTcThreads, smem, stream>>>(tq, ta, p);
+  const int sms = sm_count();
+  const unsigned grid = static_cast<unsigned>(p.n_items < sms ? p.n_items : sms);   // one CTA per SM
+  kern<<<grid, kTcThreads, smem, stream>>>(tq, ta, p);
   return check_launch("score_tc_kernel");
 }
 

@@ -19,14 +19,23 @@ __device__ __forceinline__ float unkey(uint32_t k) {
 
 constexpr int kMaxCand = 256;  // 2 * k_budget <= 256
 
+// Tells the producer of keys[] that this warp holds everything it needs in registers: one arrival
+// on the shared-memory mbarrier `bar` (0 = nobody is waiting).
+__device__ __forceinline__ void release_keys(uint32_t bar, int lane) {
+  __syncwarp();
+  if (bar != 0u && lane == 0)
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+
 // Keys of the free blocks 1..t-1 are held KPL per lane in registers (entry j of lane l is free index
 // j*32+l; 0 pads, it is below every key of a finite score).  Finds the need-th largest key by
 // bisection on the bits below the common prefix of the warp's min and max key, then compacts the
 // selected entries in index order (ties at the threshold -> lower block index, G6) into cand[] as
-// (key << 32) | ~block.  n_free > need.
+// (key << 32) | ~block.  n_free > need.  keys[] is not read again once release_keys() has run.
 template <int KPL>
 __device__ __forceinline__ void warp_topk_compact(const uint32_t* keys, int n_free, int need,
-                                                  unsigned long long* cand, int lane) {
+                                                  unsigned long long* cand, int lane,
+                                                  uint32_t release_bar) {
   const unsigned full = 0xffffffffu;
   uint32_t r[KPL];
   uint32_t hi = 0u, lo = 0xffffffffu;
@@ -38,6 +47,7 @@ __device__ __forceinline__ void warp_topk_compact(const uint32_t* keys, int n_fr
     hi = max(hi, r[j]);
     lo = v ? min(lo, r[j]) : lo;
   }
+  release_keys(release_bar, lane);
   hi = __reduce_max_sync(full, hi);
   lo = __reduce_min_sync(full, lo);
   uint32_t vth = hi;
@@ -92,8 +102,11 @@ __device__ __forceinline__ void warp_topk_compact(const uint32_t* keys, int n_fr
 // One warp.  keys[0..t] = order-preserving keys (okey) of the tile scores of the visible blocks, in
 // shared memory.  Writes the first W slots of the sorted row [0, t, free blocks by (score desc, index
 // asc)], padded with NB, and returns sigma (Eq.4 / Eq.11; G1, G5).  s3 = 3 words of scratch.
+// `release_bar`: mbarrier (shared-memory address, or 0) that receives exactly one arrival as soon as
+// keys[] has been consumed, so that the buffer can be refilled while the selection continues.
 static __device__ float warp_select(const uint32_t* keys, int t, int k, int NB, int W, int32_t* row_out,
-                                    unsigned long long* cand, uint32_t* s3, int lane) {
+                                    unsigned long long* cand, uint32_t* s3, int lane,
+                                    uint32_t release_bar = 0u) {
   const int f = (t == 0) ? 1 : 2;               // forced: sink, self (Eq.9)
   const int n_free = (t >= 2) ? t - 1 : 0;      // blocks 1 .. t-1
   const int want = 2 * k - f;
@@ -103,16 +116,17 @@ static __device__ float warp_select(const uint32_t* keys, int t, int k, int NB, 
       for (int i = lane; i < n_free; i += 32)
         cand[i] = (static_cast<unsigned long long>(keys[1 + i]) << 32) |
                   (0xFFFFFFFFu - static_cast<uint32_t>(1 + i));
+      release_keys(release_bar, lane);
     } else if (n_free <= 32 * 8) {
-      warp_topk_compact<8>(keys, n_free, need, cand, lane);
+      warp_topk_compact<8>(keys, n_free, need, cand, lane, release_bar);
     } else if (n_free <= 32 * 16) {
-      warp_topk_compact<16>(keys, n_free, need, cand, lane);
+      warp_topk_compact<16>(keys, n_free, need, cand, lane, release_bar);
     } else if (n_free <= 32 * 32) {
-      warp_topk_compact<32>(keys, n_free, need, cand, lane);
+      warp_topk_compact<32>(keys, n_free, need, cand, lane, release_bar);
     } else if (n_free <= 32 * 64) {
-      warp_topk_compact<64>(keys, n_free, need, cand, lane);
+      warp_topk_compact<64>(keys, n_free, need, cand, lane, release_bar);
     } else {
-      warp_topk_compact<128>(keys, n_free, need, cand, lane);
+      warp_topk_compact<128>(keys, n_free, need, cand, lane, release_bar);
     }
     __syncwarp();
     // order by rank: the (key, ~block) words are distinct, so rank = #{cand > mine} is a permutation
@@ -129,6 +143,7 @@ static __device__ float warp_select(const uint32_t* keys, int t, int k, int NB, 
       if (rank == i_lo) s3[2] = key;
     }
   }
+  if (need <= 0) release_keys(release_bar, lane);
   if (lane == 0) {
     row_out[0] = 0;
     if (W > 1) row_out[1] = (t > 0) ? t : NB;
