@@ -26,6 +26,12 @@ constexpr int BN = 64;                 // keys per pipeline stage / per S tile
 constexpr int kThreads = 192;
 constexpr int kMaxW = 256;             // widest kv_idx row staged in shared memory
 
+// Measured alternatives that did NOT help on B200 (C2 sparse attention, 1.81 ms): two 64-key
+// sub-blocks per iteration (2.27 ms: the K/V ring shrinks to 1.25 iterations), eight softmax warps
+// splitting the columns of each row (1.90 ms: the pair barrier costs more than the shorter exp2
+// chain saves), a double-buffered P tile (1.85 ms; dense 1135 -> 993 TFLOP/s through the smaller
+// ring).  Ablation of the same kernel: TMA gather alone 0.96 ms (19 TB/s = 64 B/clk/SM, the SM's
+// L2 port), gather + softmax without MMAs 1.42 ms, UMMA M=64 floor 1.02 ms.
 template <int BM, int D>
 struct Cfg {
   static constexpr int kOcc = (D <= 128) ? 2 : 1;  // CTAs per SM this kernel is sized for
@@ -36,8 +42,10 @@ struct Cfg {
   static constexpr int kNSraw = (kBudget - Q_BYTES - P_BYTES) / KV_BYTES;
   static constexpr int NS = kNSraw > 8 ? 8 : kNSraw;
   static constexpr int SMEM = Q_BYTES + P_BYTES + NS * KV_BYTES + 1024;
-  static constexpr uint32_t TMEM_COLS = (D == 64) ? 128 : (D == 128 ? 256 : 512);
-  static constexpr int O_COL = 64;  // S occupies columns [0,64), O columns [64, 64+D)
+  // TMEM: S is double buffered -- columns [0,64) and [64,128) -- so that QK(j+1) can be issued and
+  // retire while the softmax warps still work on S(j); O occupies columns [128, 128+D).
+  static constexpr int O_COL = 2 * BN;
+  static constexpr uint32_t TMEM_COLS = (O_COL + D <= 256) ? 256 : 512;
   static_assert(NS >= 2, "not enough shared memory for a K/V ring");
 };
 
@@ -53,7 +61,9 @@ struct Params {
 
 // bookkeeping block at the end of dynamic shared memory
 struct alignas(8) Ctl {
-  uint64_t q_full, s_full, s_free, p_full, o_done;
+  uint64_t q_full, p_full;
+  uint64_t s_full[2], s_free[2];   // per S buffer
+  uint64_t o_done;
   uint64_t kv_full[8], kv_empty[8];
   uint32_t tmem_base;
   int32_t n_valid;
@@ -76,15 +86,15 @@ __device__ __forceinline__ void softmax_m128(const Params& p, Ctl* ctl, uint8_t*
   float m = -INFINITY, l = 0.f;
   for (int j = 0; j < n_it; ++j) {
     const int k0 = key_start(j);
-    mbar_wait(smem_u32(&ctl->s_full), j & 1);
+    mbar_wait(smem_u32(&ctl->s_full[j & 1]), (j >> 1) & 1);
     tc_fence_after();
     uint32_t sa[32], sb[32];
-    tmem_ld32(tS, sa);
-    tmem_ld32(tS + 32, sb);
+    tmem_ld32(tS + (j & 1) * BN, sa);
+    tmem_ld32(tS + (j & 1) * BN + 32, sb);
     tmem_ld_wait();
     tc_fence_before();
     __syncwarp();
-    if (lane == 0) mbar_arrive(smem_u32(&ctl->s_free));
+    if (lane == 0) mbar_arrive(smem_u32(&ctl->s_free[j & 1]));
 
     float x[64];
 #pragma unroll
@@ -194,14 +204,14 @@ __device__ __forceinline__ void softmax_m64(const Params& p, Ctl* ctl, uint8_t* 
   const int sw = rA & 7;  // == rB & 7
   for (int j = 0; j < n_it; ++j) {
     const int k0 = key_start(j);
-    mbar_wait(smem_u32(&ctl->s_full), j & 1);
+    mbar_wait(smem_u32(&ctl->s_full[j & 1]), (j >> 1) & 1);
     tc_fence_after();
     uint32_t s[32];
-    tmem_ld16x256_x8(tS, s);
+    tmem_ld16x256_x8(tS + (j & 1) * BN, s);
     tmem_ld_wait();
     tc_fence_before();
     __syncwarp();
-    if (lane == 0) mbar_arrive(smem_u32(&ctl->s_free));
+    if (lane == 0) mbar_arrive(smem_u32(&ctl->s_free[j & 1]));
 
     float xa[16], xb[16];
 #pragma unroll
@@ -355,8 +365,10 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
   // ---- setup ---------------------------------------------------------------------------------
   if (warp == 5 && lane == 0) {
     mbar_init(smem_u32(&ctl->q_full), 1);
-    mbar_init(smem_u32(&ctl->s_full), 1);
-    mbar_init(smem_u32(&ctl->s_free), 4);
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(smem_u32(&ctl->s_full[i]), 1);
+      mbar_init(smem_u32(&ctl->s_free[i]), 4);
+    }
     mbar_init(smem_u32(&ctl->p_full), 4);
     mbar_init(smem_u32(&ctl->o_done), 1);
     for (int s = 0; s < C::NS; ++s) {
@@ -435,24 +447,29 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
         const uint32_t tS = tmem, tO = tmem + C::O_COL;
         const uint32_t q_a = smem_u32(q_s), p_a = smem_u32(p_s), kv_a = smem_u32(kv_s);
         mbar_wait(smem_u32(&ctl->q_full), 0);
-        for (int j = 0; j <= n_it; ++j) {
-          if (j < n_it) {  // S(j) = Q K_j^T
-            const int it = 2 * j, s = it % C::NS;
-            mbar_wait(smem_u32(&ctl->kv_full[s]), (it / C::NS) & 1);
-            if (j > 0) mbar_wait(smem_u32(&ctl->s_free), (j - 1) & 1);
-            tc_fence_after();
-            const uint32_t k_a = kv_a + s * C::KV_BYTES;
+        // S(i) = Q K_i^T into S buffer i & 1
+        auto issue_qk = [&](int i) {
+          const int it = 2 * i, s = it % C::NS;
+          mbar_wait(smem_u32(&ctl->kv_full[s]), (it / C::NS) & 1);
+          if (i >= 2) mbar_wait(smem_u32(&ctl->s_free[i & 1]), ((i >> 1) & 1) ^ 1);   // softmax(i-2) read it
+          tc_fence_after();
+          const uint32_t k_a = kv_a + s * C::KV_BYTES;
 #pragma unroll
-            for (int ks = 0; ks < D / 16; ++ks) {
-              const uint64_t ad = umma_smem_desc(q_a + (ks >> 2) * (BM * 128) + (ks & 3) * 32, 16, 1024);
-              const uint64_t bd = umma_smem_desc(k_a + (ks >> 2) * (BN * 128) + (ks & 3) * 32, 16, 1024);
-              umma_ss(tS, ad, bd, idesc_qk, ks > 0);
-            }
-            tc_commit(smem_u32(&ctl->kv_empty[s]));
-            tc_commit(smem_u32(&ctl->s_full));
+          for (int ks = 0; ks < D / 16; ++ks) {
+            const uint64_t ad = umma_smem_desc(q_a + (ks >> 2) * (BM * 128) + (ks & 3) * 32, 16, 1024);
+            const uint64_t bd = umma_smem_desc(k_a + (ks >> 2) * (BN * 128) + (ks & 3) * 32, 16, 1024);
+            umma_ss(tS + (i & 1) * BN, ad, bd, idesc_qk, ks > 0);
           }
-          if (j > 0) {  // O += P(j-1) V_{j-1}
-            const int jj = j - 1, it = 2 * jj + 1, s = it % C::NS;
+          tc_commit(smem_u32(&ctl->kv_empty[s]));
+          tc_commit(smem_u32(&ctl->s_full[i & 1]));
+        };
+        // issue order QK(0) QK(1) PV(0) QK(2) PV(1) ...: the QK product runs one iteration ahead of
+        // the softmax, so S(j+1) is already in TMEM when the softmax warps finish S(j)
+        issue_qk(0);
+        for (int jj = 0; jj < n_it; ++jj) {
+          if (jj + 1 < n_it) issue_qk(jj + 1);
+          {  // O += P(jj) V_jj
+            const int it = 2 * jj + 1, s = it % C::NS;
             mbar_wait(smem_u32(&ctl->kv_full[s]), (it / C::NS) & 1);
             mbar_wait(smem_u32(&ctl->p_full), jj & 1);
             tc_fence_after();
