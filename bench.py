@@ -451,6 +451,31 @@ def run_gpu(args):
                 torch.cuda.empty_cache()
         line["long_context"] = extra
 
+    # ---- the sweeps the paper itself varies (L123, L241-252), timing only ---------------
+    if args.sweep and world == 1:
+        from dataclasses import replace
+        try:
+            del run
+        except NameError:
+            pass
+        torch.cuda.empty_cache()
+        sweeps = {}
+        for kb, pol, qf in ([(kb, "router_quest", 0.25) for kb in (33, 40, 47, 52, 66)] +
+                            [(kb, "quest", 0.0) for kb in (33, 66)] +
+                            [(cfg.k_budget, "router_quest", qf) for qf in (0.1, 0.2, 0.3, 0.4)]):
+            c = replace(cfg, k_budget=kb)
+            r2 = Runner(c, inp, pol, qf, torch, bsa)
+            m2, _ = r2.timed_steps(3, 1, with_dense=False)
+            kvs = int(r2.sel["kv_count"].sum().item())
+            a2 = algorithmic(c, kvs)
+            sweeps[f"k={kb}/{pol}/q={qf}"] = {
+                "sparse_path_ms": m2["pool"] + m2["select"] + m2["sparse"], "select_ms": m2["select"],
+                "sparse_attn_ms": m2["sparse"], "mean_blocks_per_tile": kvs / (c.n_q_heads * c.n_blocks),
+                "sparse_tflops": a2["sparse_flops"] / (m2["sparse"] * 1e-3) / 1e12}
+            del r2
+            torch.cuda.empty_cache()
+        line["sweeps"] = sweeps
+
     # ---- CPU oracle on this host's cores --------------------------------------------------------------
     import oracle
     cpu_ms, cpu_s, text = oracle_sample_ms(cfg, inp, args.policy, args.q_frac, 16)
@@ -471,6 +496,8 @@ def main():
     ap.add_argument("--q-frac", type=float, default=0.25)
     ap.add_argument("--impl", default="bsa", choices=["bsa", "reference"])
     ap.add_argument("--no-extra", action="store_true", help="skip the 64K / 128K ratio runs")
+    ap.add_argument("--sweep", action="store_true",
+                    help="also time the k_budget / q_frac sweeps of the paper (L123, L241-252)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

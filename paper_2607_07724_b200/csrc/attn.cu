@@ -363,23 +363,24 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
   if ((smem_u32(smem) & 1023u) != 0) __trap();
 
   // ---- setup ---------------------------------------------------------------------------------
-  if (warp == 5 && lane == 0) {
-    mbar_init(smem_u32(&ctl->q_full), 1);
-    for (int i = 0; i < 2; ++i) {
-      mbar_init(smem_u32(&ctl->s_full[i]), 1);
-      mbar_init(smem_u32(&ctl->s_free[i]), 4);
-    }
-    mbar_init(smem_u32(&ctl->p_full), 4);
-    mbar_init(smem_u32(&ctl->o_done), 1);
-    for (int s = 0; s < C::NS; ++s) {
-      mbar_init(smem_u32(&ctl->kv_full[s]), 1);
-      mbar_init(smem_u32(&ctl->kv_empty[s]), 1);
-    }
-    fence_mbar_init();
-  }
   if (warp == 4) {
     if (lane == 0) {
-      tma_prefetch_desc(&tmQ);
+      mbar_init(smem_u32(&ctl->q_full), 1);
+      for (int i = 0; i < 2; ++i) {
+        mbar_init(smem_u32(&ctl->s_full[i]), 1);
+        mbar_init(smem_u32(&ctl->s_free[i]), 4);
+      }
+      mbar_init(smem_u32(&ctl->p_full), 4);
+      mbar_init(smem_u32(&ctl->o_done), 1);
+      for (int s = 0; s < C::NS; ++s) {
+        mbar_init(smem_u32(&ctl->kv_full[s]), 1);
+        mbar_init(smem_u32(&ctl->kv_empty[s]), 1);
+      }
+      fence_mbar_init();
+      // the Q tile does not depend on the kv_idx row: start it now, under the TMEM allocation and
+      // the list compaction below (both ~1 us of latency)
+      mbar_arrive_expect_tx(smem_u32(&ctl->q_full), C::Q_BYTES);
+      tma_load_5d(smem_u32(q_s), &tmQ, smem_u32(&ctl->q_full), 0, q0, 0, h, b);
       tma_prefetch_desc(&tmK);
       tma_prefetch_desc(&tmV);
     }
@@ -425,8 +426,6 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
     if (warp == 4) {
       // ---- TMA producer ----------------------------------------------------------------------
       if (lane == 0) {
-        mbar_arrive_expect_tx(smem_u32(&ctl->q_full), C::Q_BYTES);
-        tma_load_5d(smem_u32(q_s), &tmQ, smem_u32(&ctl->q_full), 0, q0, 0, h, b);
         for (int j = 0; j < n_it; ++j) {
           const int k0 = key_start(j);
 #pragma unroll
@@ -495,6 +494,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
     }
   } else if (warp < 4) {
     // nothing attended (possible only with a caller-provided kv_idx): zeros, lse = -inf
+    mbar_wait(smem_u32(&ctl->q_full), 0);   // the Q tile load must land before the CTA may exit
     const bool active = (BM == 128) || (lane < 16);
     const int r = (BM == 128) ? tid : (warp * 16 + (lane & 15));
     const int qrow = q0 + r;

@@ -3,12 +3,8 @@
 // padded kv_idx (Eq.1-5; A.2-A.9 L296-340; readings G1-G17 in DESIGN.md).
 //
 // Kernels
-//   score_select_kernel : one CTA per (tile t, head h, batch).  Tile scores of the visible blocks
-//                         (Eq.3: max over the tile's rows of Eq.1 / Eq.2) are kept in shared memory
-//                         only; warp 0 then selects the top-(2k) by a bit-wise bisection on the
-//                         order-preserving integer image of the fp32 score (ties -> lower block
-//                         index), sorts the survivors with a shared-memory bitonic network, and
-//                         emits the sorted prefix into kv_idx plus sigma (Eq.4 / Eq.11).
+//   score_tc_kernel (score_tc.cu) : tensor-core tile scores (Eq.1-3), top-(2k) and sigma (Eq.4 /
+//                         Eq.11) per (tile, head); writes all 2k / k slots of kv_idx and sigma.
 //   route_kernel        : one CTA per sequence: sigma_bar (Eq.12), device radix-select of the
 //                         ceil(qT)-th smallest sigma_bar (Eq.5 / Eq.13), trigger.
 //   finalize_kernel     : Eq.14: untriggered tiles keep k entries, the rest becomes the sentinel.
@@ -34,6 +30,7 @@ route_kernel(const float* __restrict__ sigma, int H, int T, int router, long lon
   const int b = blockIdx.x, tid = threadIdx.x;
   for (int t = tid; t < T; t += kRouteThreads) {
     float acc = 0.0f;
+#pragma unroll 8
     for (int h = 0; h < H; ++h) acc = acc + sigma[(static_cast<size_t>(b) * H + h) * T + t];  // Eq.12
     const float sb = __fdiv_rn(acc, static_cast<float>(H));
     sigma_bar[static_cast<size_t>(b) * T + t] = sb;
@@ -56,14 +53,32 @@ route_kernel(const float* __restrict__ sigma, int H, int T, int router, long lon
       if ((kk & mask) == prefix) atomicAdd(&hist[(kk >> shift) & 255u], 1u);
     }
     __syncthreads();
-    if (tid == 0) {
-      uint32_t cum = 0, d = 0;
-      for (; d < 256; ++d) {
-        if (cum + hist[d] >= remaining) break;
-        cum += hist[d];
+    if (tid < 32) {
+      // warp 0 locates the digit: 8 bins per lane, warp-inclusive scan of the lane sums, then the
+      // one lane whose range crosses `remaining` walks its 8 bins
+      uint32_t v[8], sum = 0;
+#pragma unroll
+      for (int d = 0; d < 8; ++d) {
+        v[d] = hist[tid * 8 + d];
+        sum += v[d];
       }
-      scratch[0] = d;
-      scratch[1] = remaining - cum;
+      uint32_t incl = sum;
+#pragma unroll
+      for (int off = 1; off < 32; off <<= 1) {
+        const uint32_t up = __shfl_up_sync(0xffffffffu, incl, off);
+        if (tid >= off) incl += up;
+      }
+      const unsigned hit = __ballot_sync(0xffffffffu, incl >= remaining);
+      if (tid == __ffs(hit) - 1) {
+        uint32_t cum = incl - sum;
+        int d = 0;
+        for (; d < 7; ++d) {
+          if (cum + v[d] >= remaining) break;
+          cum += v[d];
+        }
+        scratch[0] = static_cast<uint32_t>(tid * 8 + d);
+        scratch[1] = remaining - cum;
+      }
     }
     __syncthreads();
     prefix |= scratch[0] << shift;
