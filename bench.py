@@ -430,12 +430,13 @@ def run_gpu(args):
         extra = {}
         del run
         torch.cuda.empty_cache()
-        for name in ("C3a", "C3b"):
+        for name, pols in (("C3a", ("router_quest", "topk")), ("C3b", ("router_quest", "topk")),
+                           ("C4", ("router_quest", "quest")), ("C5", ("router_quest", "router"))):
             c = synth.CONFIGS[name]
             i2 = synth.make_inputs(c)
-            for pol in ("router_quest", "topk"):
+            for pol in pols:
                 r2 = Runner(c, i2, pol, args.q_frac, torch, bsa)
-                m2, _ = r2.timed_steps(3, 1, with_dense=(pol == "router_quest"))
+                m2, _ = r2.timed_steps(3, 1, with_dense=(pol == "router_quest"))   # dense once per config
                 if pol == "router_quest":
                     dense_ms = m2["dense"]
                 s = m2["pool"] + m2["select"] + m2["sparse"]

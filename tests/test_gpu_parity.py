@@ -306,3 +306,114 @@ def test_full_size_c2(bsa, policy):
         big = tt + 1 >= 2 * k                       # Eq.15 closed form on tiles that can expand fully
         qprime = trig[big].mean()
         assert abs(kvc[0, big].mean() - k * (1 + qprime)) < 1e-9
+
+
+# ---- the other BASELINE.json configs at FULL size: sampled tiles --------------------------------
+# The oracle's selection over every tile of a 128K sequence is ~1e12 MACs; O3-O7 on a stratified
+# sample of tiles (all heads) is exact for those tiles and takes seconds.  What needs every tile --
+# the quantile threshold -- is checked through properties that hold at any size.
+def _check_row(g_row, o_row, cnt, sc, t, n_blocks, what):
+    """kv_idx row against the oracle's, bit-exact or inside the 1e-5 relative tie band (north_star)."""
+    from parity_util import TIE_REL
+    assert (g_row[cnt:] == n_blocks).all(), f"{what}: padding not sentinel"
+    assert g_row[0] == 0 and (t == 0 or g_row[1] == t), f"{what}: forced blocks missing"
+    if np.array_equal(g_row[:cnt], o_row[:cnt]):
+        return False
+    gs, os_ = set(g_row[:cnt].tolist()), set(o_row[:cnt].tolist())
+    assert len(gs) == cnt and all(0 <= b <= t for b in gs), f"{what}: invalid blocks"
+    for gb, ob in zip(g_row[:cnt], o_row[:cnt]):
+        if gb != ob:
+            a, b = float(sc[gb]), float(sc[ob])
+            assert abs(a - b) <= TIE_REL * max(abs(a), abs(b)), f"{what}: blocks {gb},{ob} scores {a},{b}"
+    for blk in gs ^ os_:
+        bnd, a = float(sc[o_row[cnt - 1]]), float(sc[blk])
+        assert abs(a - bnd) <= TIE_REL * max(abs(a), abs(bnd)), f"{what}: set differs, block {blk}"
+    return True
+
+
+FULL_SAMPLED = [("C3b", "router_quest", 0.25), ("C3b", "topk", 0.25), ("C3a", "router_quest", 0.25),
+                ("C4", "quest", 0.25), ("C4", "router_quest", 0.5), ("C4", "router_quest", 0.1),
+                ("C5", "router", 0.25), ("C5", "router_quest", 0.25)]
+
+
+@pytest.mark.parametrize("name,policy,q", FULL_SAMPLED)
+def test_full_size_sampled(bsa, name, policy, q):
+    import torch
+    from parity_util import SIGMA_TOL, TIE_REL
+    cfg, inp, meta_np = _case(name)
+    Q, K, V = _dev(inp)
+    T, H, k, NB = cfg.n_blocks, cfg.n_q_heads, cfg.k_budget, cfg.n_blocks
+    router = policy.startswith("router")
+    buf = bsa.bsa_build_block_meta(K, cfg.block, 3)
+    kmean, kmin, kmax = bsa.meta_views(buf, K.shape, cfg.block)
+    assert np.array_equal(kmean[0].cpu().numpy().view(np.uint32), meta_np[0].view(np.uint32)), "kmean"
+    assert np.array_equal(bf16_to_f32(bf16_bits(kmin[0])), bf16_to_f32(meta_np[1])), "kmin"
+    assert np.array_equal(bf16_to_f32(bf16_bits(kmax[0])), bf16_to_f32(meta_np[2])), "kmax"
+    r = bsa.bsa_select(Q, buf, K, cfg.block, policy, k, q)
+    O, _ = bsa.bsa_sparse_attn_fwd(Q, K, V, r["kv_idx"], r["kv_count"], cfg.block)
+    Od, _ = bsa.bsa_dense_attn_fwd(Q, K, V, cfg.block)
+    torch.cuda.synchronize()
+    g = _gpu_select_np(r)
+    W = g["kv_idx"].shape[2]
+
+    # -- properties that hold at any size -------------------------------------------------------------
+    tt = np.arange(T)
+    trig = g["trigger"].astype(bool)
+    expect = np.minimum(np.where(trig, 2 * k, k) if router else k, tt + 1)
+    assert (g["kv_count"] == expect[None, :]).all(), "kv_count vs trigger (Eq.14)"
+    assert ((g["sigma"] >= 0) & (g["sigma"] <= 1)).all(), "sigma in [0,1]"
+    sb = g["sigma_bar"]
+    np.testing.assert_allclose(sb, g["sigma"].astype(np.float64).mean(axis=0), rtol=0, atol=1e-6)
+    if router:
+        m = int(np.ceil(q * T - 1e-9))
+        assert trig.sum() >= m and np.array_equal(trig, sb <= np.sort(sb)[m - 1]), "order-statistic trigger"
+        assert abs(g["tau"] - np.sort(sb)[m - 1]) == 0.0
+    else:
+        assert not trig.any()
+    assert (g["kv_idx"][:, :, 0] == 0).all() and (g["kv_idx"][:, 1:, 1] == tt[None, 1:]).all(), "forced"
+
+    # -- sampled tiles against the oracle ---------------------------------------------------------------
+    needle_t = sorted({n["q_row"] // cfg.block for n in inp.needles[:3]})
+    tiles = sorted(set([0, 1, 2, k - 1, k, 2 * k - 1, 2 * k, T // 4 + 3, T // 2, (3 * T) // 4 + 1, T - 2, T - 1]
+                       + needle_t))
+    tiles = [t for t in tiles if 0 <= t < T]
+    orc = oracle.select_tiles(inp.Q, meta_np, cfg.block, policy, k, tiles, want_scores=True)
+    kv_full = np.full((H, T, W), NB, np.int32)
+    cnt_full = np.zeros((H, T), np.int32)
+    ties, sig_ties, clean = 0, 0, []
+    for i, t in enumerate(tiles):
+        cnt = int(expect[t])
+        for h in range(H):
+            o_row = orc["idx_sorted"][i, h]
+            kv_full[h, t, :cnt] = o_row[:cnt]
+            cnt_full[h, t] = cnt
+            tie = _check_row(g["kv_idx"][h, t], o_row, cnt, orc["tile_score"][i, h], t, NB,
+                             f"{name}/{policy} h={h} t={t}")
+            ties += tie
+            if not tie:
+                clean.append((t, h))
+            ds = abs(float(g["sigma"][h, t]) - float(orc["sigma"][i, h]))
+            if ds > SIGMA_TOL:
+                ss = orc["score_sorted"][i, h]
+                f = 1 if t == 0 else 2
+                den = float(ss[f]) - float(ss[k])
+                scale = max(abs(float(ss[f])), abs(float(ss[k])))
+                assert den <= 100 * TIE_REL * scale, f"sigma h={h} t={t}: {g['sigma'][h, t]} vs {orc['sigma'][i, h]}"
+                sig_ties += 1
+        assert abs(float(sb[t]) - float(orc["sigma"][i].astype(np.float32).mean())) <= SIGMA_TOL, "sigma_bar"
+    assert ties <= max(2, len(tiles) * H // 50), f"{ties} tie rows in {len(tiles) * H}"
+    _log(f"{name}/{policy}/q={q}", dict(stage="full-sampled", rows=len(tiles) * H, tie_rows=ties,
+                                        sigma_tie_rows=sig_ties))
+
+    # -- attention on sampled (tile, head) pairs, kv_idx rows from the ORACLE -----------------------------
+    heads = sorted({0, H // 2, H - 1})
+    pairs = [(t, h) for t in tiles for h in heads if (t, h) in set(clean)][:24]
+    ref, _ = oracle.attn_pairs(inp.Q, inp.K, inp.V, cfg.block, pairs, kv_full, cnt_full)
+    Og = O[0].float().cpu().numpy().reshape(H, T, cfg.block, cfg.head_dim)
+    compare_attn(np.stack([Og[h, t] for t, h in pairs]), ref, f"{name} sparse {policy}")
+    dpairs = [(0, 0), (1, H - 1), (T // 8, H // 2)]
+    refd, _ = oracle.attn_pairs(inp.Q, inp.K, inp.V, cfg.block, dpairs)
+    Odg = Od[0].float().cpu().numpy().reshape(H, T, cfg.block, cfg.head_dim)
+    compare_attn(np.stack([Odg[h, t] for t, h in dpairs]), refd, f"{name} dense")
+    del Q, K, V, O, Od, r
+    torch.cuda.empty_cache()
