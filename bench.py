@@ -199,6 +199,18 @@ def workload_config(cfg, args):
             "parallelism": "replicas only"}
 
 
+def max_over_ranks(values, world: int, device: str):
+    """Replicas only: every rank times the same independent workload; a multi-GPU
+    number is the MAX over ranks of the device-timed milliseconds.  No data-path collective exists."""
+    if world <= 1:
+        return [float(v) for v in values]
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(v) for v in values], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t.tolist()]
+
+
 # ---- the GPU arm ----------------------------------------------------------------------------------
 class Runner:
     """Device tensors + preallocated outputs for one workload; step() enqueues rows 1-7."""
@@ -359,19 +371,12 @@ def run_gpu(args):
 
     sparse_ms = mean["pool"] + mean["select"] + mean["sparse"]
     step_ms = sparse_ms + mean["dense"]
-    if world > 1:
-        t = torch.tensor([sparse_ms, step_ms, mean["sparse"], mean["dense"]], device="cuda",
-                         dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        sparse_ms, step_ms = float(t[0]), float(t[1])
+    sparse_ms, step_ms = max_over_ranks([sparse_ms, step_ms], world, "cuda")
 
     kv_sum = int(run.sel["kv_count"].sum().item())
     alg = algorithmic(cfg, kv_sum)
     e2e_ms, h2d, d2h = run.e2e_steps(max(2, min(args.steps, 5)), 2)
-    if world > 1:
-        t = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t[0])
+    (e2e_ms,) = max_over_ranks([e2e_ms], world, "cuda")
 
     if rank != 0:
         if world > 1:
