@@ -3,13 +3,13 @@
 // kv_idx with a single-compare sentinel skip), and the dense causal kernel of the same design
 // (L45, L156) used as the "x dense" denominator.
 //
-// One CTA per (Q tile, head, batch); 6 warps:
+// One CTA per (Q tile, head, batch); 7 warps:
 //   warps 0-3  softmax: tcgen05.ld of S, fp32 online softmax in base 2, P (bf16) -> shared memory,
 //              lazy rescale of the O accumulator in TMEM, final normalisation and store
 //   warp 4     TMA producer: Q once, then K and V 64-key sub-blocks through a ring of stages; the
 //              row coordinate of each load is kv_idx * block ("gather" = ordinary tiled TMA loads)
-//   warp 5     one thread issues tcgen05.mma: S = Q K^T (both K-major, 128B swizzle) into TMEM and
-//              O += P V (V is the MN-major B operand) into TMEM
+//   warp 5     one thread issues the S = Q K^T MMAs (both operands K-major, 128B swizzle) into TMEM
+//   warp 6     one thread issues the O += P V MMAs (V is the MN-major B operand) into TMEM
 // Q tile rows: sparse = one selection tile (BM = block), dense = 128.  For BM = 64 the accumulator
 // rows live in lanes 0-15 of each TMEM sub-partition (UMMA M = 64 layout).
 #include <cuda_bf16.h>
@@ -23,7 +23,7 @@ namespace bsa {
 namespace {
 
 constexpr int BN = 64;                 // keys per pipeline stage / per S tile
-constexpr int kThreads = 192;
+constexpr int kThreads = 224;          // warps 0-3 softmax, 4 TMA, 5 QK issuer, 6 PV issuer
 constexpr int kMaxW = 256;             // widest kv_idx row staged in shared memory
 
 // Measured alternatives that did NOT help on B200 (C2 sparse attention, 1.81 ms): two 64-key
@@ -438,15 +438,21 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
           }
         }
       }
-    } else if (warp == 5) {
-      // ---- MMA issuer ------------------------------------------------------------------------
-      if (lane == 0) {
+    } else if (warp == 5 || warp == 6) {
+      // ---- MMA issue.  QK(i): S(i) = Q K_i^T into S buffer i & 1, one iteration ahead of the
+      // softmax; PV(jj): O += P(jj) V_jj.  For BM = 64 the two products are issued by TWO threads
+      // (warp 5: QK, warp 6: PV): tcgen05.mma issue blocks while the pipe is busy and every
+      // mbarrier poll costs a lone thread ~100 clk, so in one thread the waits and the issue of
+      // both products added up to the whole iteration (clock64 trace: 420 clk of waits + 1100 clk of
+      // issue per 1700-clk iteration).  The streams are independent: S vs O in TMEM, own ring
+      // slots, own commits.  For BM = 128 one thread issuing QK(j+1), PV(j) alternately measured
+      // 4 % faster and is kept.
+      constexpr bool kSplit = (BM == 64);
+      if (lane == 0 && (warp == 5 || kSplit)) {
         constexpr uint32_t idesc_qk = umma_idesc_bf16(BM, BN, 0, 0);
         constexpr uint32_t idesc_pv = umma_idesc_bf16(BM, D, 0, 1);
         const uint32_t tS = tmem, tO = tmem + C::O_COL;
         const uint32_t q_a = smem_u32(q_s), p_a = smem_u32(p_s), kv_a = smem_u32(kv_s);
-        mbar_wait(smem_u32(&ctl->q_full), 0);
-        // S(i) = Q K_i^T into S buffer i & 1
         auto issue_qk = [&](int i) {
           const int it = 2 * i, s = it % C::NS;
           mbar_wait(smem_u32(&ctl->kv_full[s]), (it / C::NS) & 1);
@@ -462,29 +468,39 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
           tc_commit(smem_u32(&ctl->kv_empty[s]));
           tc_commit(smem_u32(&ctl->s_full[i & 1]));
         };
-        // issue order QK(0) QK(1) PV(0) QK(2) PV(1) ...: the QK product runs one iteration ahead of
-        // the softmax, so S(j+1) is already in TMEM when the softmax warps finish S(j)
-        issue_qk(0);
-        for (int jj = 0; jj < n_it; ++jj) {
-          if (jj + 1 < n_it) issue_qk(jj + 1);
-          {  // O += P(jj) V_jj
-            const int it = 2 * jj + 1, s = it % C::NS;
-            mbar_wait(smem_u32(&ctl->kv_full[s]), (it / C::NS) & 1);
-            mbar_wait(smem_u32(&ctl->p_full), jj & 1);
-            tc_fence_after();
-            const uint32_t v_a = kv_a + s * C::KV_BYTES;
+        auto issue_pv = [&](int jj) {
+          const int it = 2 * jj + 1, s = it % C::NS;
+          mbar_wait(smem_u32(&ctl->kv_full[s]), (it / C::NS) & 1);
+          mbar_wait(smem_u32(&ctl->p_full), jj & 1);
+          tc_fence_after();
+          const uint32_t v_a = kv_a + s * C::KV_BYTES;
 #pragma unroll
-            for (int ks = 0; ks < BN / 16; ++ks) {
-              const uint64_t ad = umma_smem_desc(p_a + ks * 32, 16, 1024);
-              const uint64_t bd = umma_smem_desc(v_a + ks * 2048, BN * 128, 1024);
-              umma_ss(tO, ad, bd, idesc_pv, (jj > 0) || (ks > 0));
-            }
-            tc_commit(smem_u32(&ctl->kv_empty[s]));
-            tc_commit(smem_u32(&ctl->o_done));
+          for (int ks = 0; ks < BN / 16; ++ks) {
+            const uint64_t ad = umma_smem_desc(p_a + ks * 32, 16, 1024);
+            const uint64_t bd = umma_smem_desc(v_a + ks * 2048, BN * 128, 1024);
+            umma_ss(tO, ad, bd, idesc_pv, (jj > 0) || (ks > 0));
+          }
+          tc_commit(smem_u32(&ctl->kv_empty[s]));
+          tc_commit(smem_u32(&ctl->o_done));
+        };
+        if (kSplit) {
+          if (warp == 5) {
+            mbar_wait(smem_u32(&ctl->q_full), 0);
+            for (int i = 0; i < n_it; ++i) issue_qk(i);
+          } else {
+            for (int jj = 0; jj < n_it; ++jj) issue_pv(jj);
+          }
+        } else {
+          // issue order QK(0) QK(1) PV(0) QK(2) PV(1) ...
+          mbar_wait(smem_u32(&ctl->q_full), 0);
+          issue_qk(0);
+          for (int jj = 0; jj < n_it; ++jj) {
+            if (jj + 1 < n_it) issue_qk(jj + 1);
+            issue_pv(jj);
           }
         }
       }
-    } else {
+    } else if (warp < 4) {
       // ---- softmax warps ---------------------------------------------------------------------
       if constexpr (BM == 64) {
         softmax_m64<D, SPARSE>(p, ctl, p_s, tmem, n_it, q0, b, h, key_start);
