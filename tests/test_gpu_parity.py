@@ -193,6 +193,28 @@ def test_sparse_attention_parity_stagewise(bsa, name, policy):
     np.testing.assert_allclose(got_lse, ref_lse, rtol=0, atol=2e-3)
 
 
+@pytest.mark.parametrize("name,policy,reps", [("C2", "router_quest", 60), ("C3b", "topk", 40)])
+def test_sparse_attention_is_deterministic(bsa, name, policy, reps):
+    """Repeated launches on the same inputs must give bit-identical outputs.  (A build that issued the
+    QK and PV MMAs from two threads passed the parity tests but, over tens of launches at C3b/topk,
+    returned different bits in a few of them and occasionally lost an mbarrier arrival; this test is
+    the guard against that class of race.)"""
+    import torch
+    cfg, inp, _ = _case(name)
+    Q, K, V = _dev(inp)
+    buf = bsa.bsa_build_block_meta(K, cfg.block, 3)
+    r = bsa.bsa_select(Q, buf, K, cfg.block, policy, cfg.k_budget, 0.25)
+    first = None
+    for i in range(reps):
+        O, lse = bsa.bsa_sparse_attn_fwd(Q, K, V, r["kv_idx"], r["kv_count"], cfg.block, want_lse=True)
+        torch.cuda.synchronize()
+        if first is None:
+            first = (O.clone(), lse.clone())
+        else:
+            assert torch.equal(O.view(torch.int16), first[0].view(torch.int16)), f"launch {i}: O differs"
+            assert torch.equal(lse, first[1]), f"launch {i}: lse differs"
+
+
 def test_sparse_attention_edge_cases(bsa):
     """permuted rows, sentinel / future entries skipped, kv_count = NULL, empty rows -> zeros,
     k_budget >= N_B reduces to dense."""
