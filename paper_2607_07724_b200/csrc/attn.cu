@@ -3,13 +3,14 @@
 // kv_idx with a single-compare sentinel skip), and the dense causal kernel of the same design
 // (L45, L156) used as the "x dense" denominator.
 //
-// One CTA per (Q tile, head, batch); 6 warps:
+// One CTA per (Q tile, head, batch); 7 warps:
 //   warps 0-3  softmax: tcgen05.ld of S, fp32 online softmax in base 2, P (bf16) -> shared memory,
 //              lazy rescale of the O accumulator in TMEM, final normalisation and store
 //   warp 4     TMA producer: Q once, then K and V 64-key sub-blocks through a ring of stages; the
 //              row coordinate of each load is kv_idx * block ("gather" = ordinary tiled TMA loads)
-//   warp 5     one thread issues tcgen05.mma: S = Q K^T (both K-major, 128B swizzle) into TMEM and
-//              O += P V (V is the MN-major B operand) into TMEM
+//   warp 5     one thread issues tcgen05.mma: S = Q K^T (both K-major, 128B swizzle) into TMEM and,
+//              for BM = 128, O += P V (V is the MN-major B operand) into TMEM
+//   warp 6     BM = 64 only: a second thread issues the O += P V MMAs (own K/V ring, see below)
 // Q tile rows: sparse = one selection tile (BM = block), dense = 128.  For BM = 64 the accumulator
 // rows live in lanes 0-15 of each TMEM sub-partition (UMMA M = 64 layout).
 #include <cuda_bf16.h>
@@ -23,7 +24,7 @@ namespace bsa {
 namespace {
 
 constexpr int BN = 64;                 // keys per pipeline stage / per S tile
-constexpr int kThreads = 192;          // warps 0-3 softmax, 4 TMA producer, 5 MMA issuer
+constexpr int kThreads = 224;          // warps 0-3 softmax, 4 TMA, 5 MMA issuer (QK), 6 PV issuer (BM = 64)
 constexpr int kMaxW = 256;             // widest kv_idx row staged in shared memory
 
 // Measured alternatives that did NOT help on B200 (C2 sparse attention, 1.81 ms): two 64-key
@@ -46,7 +47,7 @@ struct Cfg {
   // retire while the softmax warps still work on S(j); O occupies columns [128, 128+D).
   static constexpr int O_COL = 2 * BN;
   static constexpr uint32_t TMEM_COLS = (O_COL + D <= 256) ? 256 : 512;
-  static_assert(NS >= 2, "not enough shared memory for a K/V ring");
+  static_assert(NS >= 2 && (BM != 64 || NS >= 4), "not enough shared memory for a K/V ring");
 };
 
 struct Params {
@@ -422,50 +423,59 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
     return j * BN;
   };
 
-  // ring position of K(i) and V(j) (see the producer): K leads V by kAhead iterations
-  constexpr int kAhead = 1;
+  // ---- K/V ring bookkeeping --------------------------------------------------------------------
+  // BM = 128: one thread issues QK(j+1), PV(j) alternately (kAhead = 1) and the K and V tiles share
+  // ONE ring, entered in the order that thread consumes them: K(0), then [K(j+1), V(j)].
+  // BM = 64: QK and PV are issued by TWO threads and QK runs up to two iterations ahead, so K and V
+  // get SEPARATE rings (NSK + NSV = NS slots), each with a single in-order consumer.  Sharing one
+  // ring between two consumers is a bug, not an optimisation: a parity wait on a slot's `full`
+  // barrier also succeeds when the slot's PREVIOUS occupant (the other thread's tile) has not even
+  // landed yet, so the faster thread runs MMAs on stale bytes and releases a slot it does not own
+  // (seen as non-deterministic outputs, lost arrivals and launch failures in stress runs).
+  constexpr bool kSplit = (BM == 64);
+  constexpr int kAhead = kSplit ? 2 : 1;
+  constexpr int NSK = kSplit ? (C::NS + 1) / 2 : C::NS;
+  constexpr int NSV = kSplit ? C::NS - NSK : C::NS;
   auto pos_k = [&](int i) -> int { return i < kAhead ? i : 2 * i - kAhead; };
   auto pos_v = [&](int j) -> int { const int a = 2 * j + kAhead + 1, t = j + n_it; return a < t ? a : t; };
+  auto seq_k = [&](int i) -> int { return kSplit ? i : pos_k(i); };          // index in its ring
+  auto seq_v = [&](int j) -> int { return kSplit ? j : pos_v(j); };
+  auto slot_k = [&](int i) -> int { return seq_k(i) % NSK; };
+  auto slot_v = [&](int j) -> int { return kSplit ? NSK + j % NSV : pos_v(j) % NSV; };
 
   if (n_it > 0) {
     if (warp == 4) {
-      // ---- TMA producer ----------------------------------------------------------------------
-      // Tiles enter the ring in the order the MMA threads consume them -- K runs kAhead iterations
-      // ahead of V (QK(j+kAhead) is issued before PV(j)) -- so a slot is never parked behind one
-      // that is released later:  K(0..kAhead-1), then [K(j+kAhead), V(j)] for j = 0, 1, ...
+      // ---- TMA producer: K(0..kAhead-1), then [K(j+kAhead), V(j)] for j = 0, 1, ... -------------
       if (lane == 0) {
-        int it = 0;
-        auto load = [&](const CUtensorMap* tm, int j) {
-          const int s = it % C::NS;
-          mbar_wait(smem_u32(&ctl->kv_empty[s]), ((it / C::NS) & 1) ^ 1);
+        auto load = [&](const CUtensorMap* tm, int j, int s, int seq, int ns) {
+          mbar_wait(smem_u32(&ctl->kv_empty[s]), ((seq / ns) & 1) ^ 1);
           mbar_arrive_expect_tx(smem_u32(&ctl->kv_full[s]), C::KV_BYTES);
           tma_load_5d(smem_u32(kv_s + s * C::KV_BYTES), tm, smem_u32(&ctl->kv_full[s]), 0,
                       key_start(j), 0, g, b);
-          ++it;
         };
-        for (int i = 0; i < kAhead && i < n_it; ++i) load(&tmK, i);
+        for (int i = 0; i < kAhead && i < n_it; ++i) load(&tmK, i, slot_k(i), seq_k(i), NSK);
         for (int j = 0; j < n_it; ++j) {
-          if (j + kAhead < n_it) load(&tmK, j + kAhead);
-          load(&tmV, j);
+          const int i = j + kAhead;
+          if (i < n_it) load(&tmK, i, slot_k(i), seq_k(i), NSK);
+          load(&tmV, j, slot_v(j), seq_v(j), NSV);
         }
       }
-    } else if (warp == 5) {
-      // ---- MMA issue: ONE thread issues every tcgen05.mma of the CTA.  QK(i): S(i) = Q K_i^T into S
-      // buffer i & 1, one iteration ahead of the softmax; PV(jj): O += P(jj) V_jj.  Issue order
-      // QK(0) QK(1) PV(0) QK(2) PV(1) ...
-      // A variant with QK and PV issued by two threads (warps 5 and 6) was 10 % faster but is NOT
-      // safe on B200: a 60-launch stress run at C3b/topk gave non-deterministic outputs (max diff
-      // ~0.1 in a few launches), an occasional lost mbarrier arrival and launch failures, also with
-      // the two threads' issue groups serialised by a lock; this single-thread form was bit-stable
-      // over 500 launches.
-      if (lane == 0) {
+    } else if (warp == 5 || warp == 6) {
+      // ---- MMA issue.  QK(i): S(i) = Q K_i^T into S buffer i & 1, ahead of the softmax; PV(jj):
+      // O += P(jj) V_jj.  BM = 64: issued by two threads (warp 5: QK, warp 6: PV) -- tcgen05.mma
+      // issue blocks while the pipe is busy and every mbarrier poll costs a lone thread ~100 clk, so
+      // in one thread the waits and the issue of both products added up to the whole iteration
+      // (clock64 trace: 420 clk of waits + 1100 clk of issue per 1700-clk iteration).  The two
+      // streams share nothing: S vs O in TMEM, own rings, own commits.  BM = 128: one thread,
+      // order QK(0) QK(1) PV(0) QK(2) PV(1) ... (measured 4 % faster there).
+      if (lane == 0 && (warp == 5 || kSplit)) {
         constexpr uint32_t idesc_qk = umma_idesc_bf16(BM, BN, 0, 0);
         constexpr uint32_t idesc_pv = umma_idesc_bf16(BM, D, 0, 1);
         const uint32_t tS = tmem, tO = tmem + C::O_COL;
         const uint32_t q_a = smem_u32(q_s), p_a = smem_u32(p_s), kv_a = smem_u32(kv_s);
         auto issue_qk = [&](int i) {
-          const int it = pos_k(i), s = it % C::NS;
-          mbar_wait(smem_u32(&ctl->kv_full[s]), (it / C::NS) & 1);
+          const int s = slot_k(i);
+          mbar_wait(smem_u32(&ctl->kv_full[s]), (seq_k(i) / NSK) & 1);
           if (i >= 2) mbar_wait(smem_u32(&ctl->s_free[i & 1]), ((i >> 1) & 1) ^ 1);   // softmax(i-2) read it
           tc_fence_after();
           const uint32_t k_a = kv_a + s * C::KV_BYTES;
@@ -479,8 +489,8 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
           tc_commit(smem_u32(&ctl->s_full[i & 1]));
         };
         auto issue_pv = [&](int jj) {
-          const int it = pos_v(jj), s = it % C::NS;
-          mbar_wait(smem_u32(&ctl->kv_full[s]), (it / C::NS) & 1);
+          const int s = slot_v(jj);
+          mbar_wait(smem_u32(&ctl->kv_full[s]), (seq_v(jj) / NSV) & 1);
           mbar_wait(smem_u32(&ctl->p_full), jj & 1);
           tc_fence_after();
           const uint32_t v_a = kv_a + s * C::KV_BYTES;
@@ -493,11 +503,20 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
           tc_commit(smem_u32(&ctl->kv_empty[s]));
           tc_commit(smem_u32(&ctl->o_done));
         };
-        mbar_wait(smem_u32(&ctl->q_full), 0);
-        issue_qk(0);
-        for (int jj = 0; jj < n_it; ++jj) {
-          if (jj + 1 < n_it) issue_qk(jj + 1);
-          issue_pv(jj);
+        if (kSplit) {
+          if (warp == 5) {
+            mbar_wait(smem_u32(&ctl->q_full), 0);
+            for (int i = 0; i < n_it; ++i) issue_qk(i);
+          } else {
+            for (int jj = 0; jj < n_it; ++jj) issue_pv(jj);
+          }
+        } else {
+          mbar_wait(smem_u32(&ctl->q_full), 0);
+          issue_qk(0);
+          for (int jj = 0; jj < n_it; ++jj) {
+            if (jj + 1 < n_it) issue_qk(jj + 1);
+            issue_pv(jj);
+          }
         }
       }
     } else if (warp < 4) {
