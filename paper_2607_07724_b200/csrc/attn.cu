@@ -9,8 +9,8 @@
 //   warp 4     TMA producer: Q once, then K and V 64-key sub-blocks through a ring of stages; the
 //              row coordinate of each load is kv_idx * block ("gather" = ordinary tiled TMA loads)
 //   warp 5     one thread issues tcgen05.mma: S = Q K^T (both K-major, 128B swizzle) into TMEM and,
-//              for BM = 128, O += P V (V is the MN-major B operand) into TMEM
-//   warp 6     BM = 64 only: a second thread issues the O += P V MMAs (own K/V ring, see below)
+//              for BM = 128 with d <= 128, O += P V (V is the MN-major B operand) into TMEM
+//   warp 6     BM = 64 and d = 256: a second thread issues the O += P V MMAs (own V ring, see below)
 // Q tile rows: sparse = one selection tile (BM = block), dense = 128.  For BM = 64 the accumulator
 // rows live in lanes 0-15 of each TMEM sub-partition (UMMA M = 64 layout).
 #include <cuda_bf16.h>
@@ -27,12 +27,17 @@ constexpr int BN = 64;                 // keys per pipeline stage / per S tile
 constexpr int kThreads = 224;          // warps 0-3 softmax, 4 TMA, 5 MMA issuer (QK), 6 PV issuer (BM = 64)
 constexpr int kMaxW = 256;             // widest kv_idx row staged in shared memory
 
-// Measured alternatives that did NOT help on B200 (C2 sparse attention, 1.81 ms): two 64-key
-// sub-blocks per iteration (2.27 ms: the K/V ring shrinks to 1.25 iterations), eight softmax warps
-// splitting the columns of each row (1.90 ms: the pair barrier costs more than the shorter exp2
-// chain saves), a double-buffered P tile (1.85 ms; dense 1135 -> 993 TFLOP/s through the smaller
-// ring).  Ablation of the same kernel: TMA gather alone 0.96 ms (19 TB/s = 64 B/clk/SM, the SM's
-// L2 port), gather + softmax without MMAs 1.42 ms, UMMA M=64 floor 1.02 ms.
+// Measured alternatives that did NOT help on B200 (C2 sparse attention; 1.81 ms with one issuing
+// thread, 1.53 ms with two): two 64-key sub-blocks per iteration (2.27 ms: the K/V ring shrinks to
+// 1.25 iterations), eight softmax warps splitting the columns of each row (1.90 ms: the pair barrier
+// costs more than the shorter exp2 chain saves), a double-buffered P tile (1.85 ms with one issuing
+// thread, 1.60 vs 1.53 ms with two), K:V slot splits 3:2 / 2:3 and K running 1 / 2 / 3 iterations
+// ahead (all 1.53-1.55 ms), and the transposed PV product O^T += V^T P^T (M = d = 128, N = 64: 48 clk
+// per MMA against 64 for M = 64, N = 128, see sm100_ptx.cuh; parity green but 1.80 ms -- the O
+// accumulator then has d on lanes, so the lazy rescale needs a CTA-wide vote every iteration and the
+// epilogue a transpose through shared memory).  Ablation of the same kernel: TMA gather alone
+// 0.96 ms (19 TB/s = 64 B/clk/SM, the SM's L2 port), gather + softmax without MMAs 1.42 ms, UMMA
+// M=64 floor 1.02 ms (8 x 32 + 4 x 64 clk per block with two CTAs interleaved on the pipe).
 template <int BM, int D>
 struct Cfg {
   static constexpr int kOcc = (D <= 128) ? 2 : 1;  // CTAs per SM this kernel is sized for
@@ -47,7 +52,7 @@ struct Cfg {
   // retire while the softmax warps still work on S(j); O occupies columns [128, 128+D).
   static constexpr int O_COL = 2 * BN;
   static constexpr uint32_t TMEM_COLS = (O_COL + D <= 256) ? 256 : 512;
-  static_assert(NS >= 2 && (BM != 64 || NS >= 4), "not enough shared memory for a K/V ring");
+  static_assert(NS >= 2 && ((BM != 64 && kOcc != 1) || NS >= 4), "not enough shared memory for a K/V ring");
 };
 
 struct Params {
@@ -424,15 +429,17 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
   };
 
   // ---- K/V ring bookkeeping --------------------------------------------------------------------
-  // BM = 128: one thread issues QK(j+1), PV(j) alternately (kAhead = 1) and the K and V tiles share
-  // ONE ring, entered in the order that thread consumes them: K(0), then [K(j+1), V(j)].
-  // BM = 64: QK and PV are issued by TWO threads and QK runs up to two iterations ahead, so K and V
+  // BM = 128, d <= 128 (two CTAs per SM): one thread issues QK(j+1), PV(j) alternately (kAhead = 1)
+  // and the K and V tiles share ONE ring, entered in the order that thread consumes them: K(0), then
+  // [K(j+1), V(j)].  (Two threads measured 3 % slower there: 1168 -> 1135 TFLOP/s dense at 32K.)
+  // BM = 64, and d = 256 (one CTA per SM; dense 1023 -> 1211 TFLOP/s, sparse C5 1014 -> 1145 with two
+  // threads): QK and PV are issued by TWO threads and QK runs up to two iterations ahead, so K and V
   // get SEPARATE rings (NSK + NSV = NS slots), each with a single in-order consumer.  Sharing one
   // ring between two consumers is a bug, not an optimisation: a parity wait on a slot's `full`
   // barrier also succeeds when the slot's PREVIOUS occupant (the other thread's tile) has not even
   // landed yet, so the faster thread runs MMAs on stale bytes and releases a slot it does not own
   // (seen as non-deterministic outputs, lost arrivals and launch failures in stress runs).
-  constexpr bool kSplit = (BM == 64);
+  constexpr bool kSplit = (BM == 64) || (C::kOcc == 1);
   constexpr int kAhead = kSplit ? 2 : 1;
   constexpr int NSK = kSplit ? (C::NS + 1) / 2 : C::NS;
   constexpr int NSV = kSplit ? C::NS - NSK : C::NS;
@@ -462,11 +469,11 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
       }
     } else if (warp == 5 || warp == 6) {
       // ---- MMA issue.  QK(i): S(i) = Q K_i^T into S buffer i & 1, ahead of the softmax; PV(jj):
-      // O += P(jj) V_jj.  BM = 64: issued by two threads (warp 5: QK, warp 6: PV) -- tcgen05.mma
+      // O += P(jj) V_jj.  kSplit: issued by two threads (warp 5: QK, warp 6: PV) -- tcgen05.mma
       // issue blocks while the pipe is busy and every mbarrier poll costs a lone thread ~100 clk, so
       // in one thread the waits and the issue of both products added up to the whole iteration
       // (clock64 trace: 420 clk of waits + 1100 clk of issue per 1700-clk iteration).  The two
-      // streams share nothing: S vs O in TMEM, own rings, own commits.  BM = 128: one thread,
+      // streams share nothing: S vs O in TMEM, own rings, own commits.  Otherwise: one thread,
       // order QK(0) QK(1) PV(0) QK(2) PV(1) ... (measured 4 % faster there).
       if (lane == 0 && (warp == 5 || kSplit)) {
         constexpr uint32_t idesc_qk = umma_idesc_bf16(BM, BN, 0, 0);
