@@ -280,6 +280,61 @@ def test_end_to_end_chain(bsa, name, policy):
     _log(f"{name}/{policy}", dict(stage="e2e", **stats))
 
 
+# ---- batch > 1 and token-major ([B, N, H, d]) storage --------------------------------
+@pytest.mark.parametrize("policy", ["router", "router_quest"])
+def test_batch2_token_major_layout(bsa, policy):
+    """Two different sequences in one call, Q/K/V/O stored token-major and passed as strided
+    [B, H, N, d] views: every sequence must match ITS OWN oracle run -- selection, the per-sequence
+    quantile (reading G9) and attention."""
+    import dataclasses
+    import torch
+    cfg, inp0, meta0 = _case("C2s")
+    key = "C2s/number+40"
+    if key not in _CACHE:
+        cfg1 = dataclasses.replace(cfg, number=cfg.number + 40)
+        inp1 = synth.make_inputs(cfg1)
+        _CACHE[key] = (cfg1, inp1, oracle.pool(inp1.K, cfg.block))
+    _, inp1, meta1 = _CACHE[key]
+    seqs = [(inp0, meta0), (inp1, meta1)]
+
+    def tok_major(xs):   # list of [H, N, d] bit arrays -> [B, H, N, d] view of a [B, N, H, d] buffer
+        t = torch.stack([to_torch_bf16(x) for x in xs])            # [B, H, N, d]
+        return t.permute(0, 2, 1, 3).contiguous().permute(0, 2, 1, 3)
+
+    Q, K, V = (tok_major([getattr(i, n) for i, _ in seqs]) for n in "QKV")
+    assert not Q.is_contiguous() and Q.stride(3) == 1
+    buf = bsa.bsa_build_block_meta(K, cfg.block, 3)
+    r = bsa.bsa_select(Q, buf, K, cfg.block, policy, cfg.k_budget, 0.25)
+    O, _ = bsa.bsa_sparse_attn_fwd(Q, K, V, r["kv_idx"], r["kv_count"], cfg.block)
+    Od, _ = bsa.bsa_dense_attn_fwd(Q, K, V, cfg.block)
+    torch.cuda.synchronize()
+    assert O.stride() == Q.stride()
+    T, H = cfg.n_blocks, cfg.n_q_heads
+    taus = []
+    for bi, (inp, meta_np) in enumerate(seqs):
+        kmean, _, _ = bsa.meta_views(buf, K.shape, cfg.block)
+        assert np.array_equal(kmean[bi].cpu().numpy().view(np.uint32), meta_np[0].view(np.uint32))
+        orc = oracle.select(inp.Q, meta_np, cfg.block, policy, cfg.k_budget, 0.25, want_scores=True)
+        g = dict(kv_idx=r["kv_idx"][bi].cpu().numpy(), kv_count=r["kv_count"][bi].cpu().numpy(),
+                 sigma=r["sigma"][bi].cpu().numpy(), sigma_bar=r["sigma_bar"][bi].cpu().numpy(),
+                 trigger=r["trigger"][bi].cpu().numpy(), tau=float(r["tau"][bi].item()))
+        log = []
+        stats = compare_select(g, orc, cfg.n_blocks, cfg.k_budget, log)
+        _log(f"C2s-batch2[{bi}]/{policy}", dict(stage="batch2", **stats))
+        taus.append(g["tau"])
+        tied = {(e[1], e[2]) for e in log if e[0] == "kv_idx"}
+        flipped_t = {e[1] for e in log if e[0] == "trigger"}
+        pairs = [(t, h) for h in (0, H - 1) for t in (0, 1, cfg.k_budget, T // 2, T - 1)
+                 if (h, t) not in tied and t not in flipped_t]
+        ref, _ = oracle.attn_pairs(inp.Q, inp.K, inp.V, cfg.block, pairs, orc["kv_idx"], orc["kv_count"])
+        Og = O[bi].float().cpu().numpy().reshape(H, T, cfg.block, cfg.head_dim)
+        compare_attn(np.stack([Og[h, t] for t, h in pairs]), ref, f"batch2[{bi}] sparse {policy}")
+        refd, _ = oracle.attn_pairs(inp.Q, inp.K, inp.V, cfg.block, pairs)
+        Odg = Od[bi].float().cpu().numpy().reshape(H, T, cfg.block, cfg.head_dim)
+        compare_attn(np.stack([Odg[h, t] for t, h in pairs]), refd, f"batch2[{bi}] dense")
+    assert taus[0] != taus[1], "the quantile threshold is per sequence (G9)"
+
+
 # ---- BASELINE.json configs[1] at full size, the launch configuration bench.py times --------------
 @pytest.mark.parametrize("policy", ["router_quest", "topk"])
 def test_full_size_c2(bsa, policy):
