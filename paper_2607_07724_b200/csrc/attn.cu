@@ -120,15 +120,22 @@ __device__ __forceinline__ void softmax_m128(const Params& p, Ctl* ctl, uint8_t*
     const bool any = __any_sync(0xffffffffu, m_new - m > 8.0f);
     if (!any) m_new = m;
     const float alpha = ex2_approx(m - m_new);
-    float sum = 0.f;
+    // packed fp32x2 FMA / ADD (FFMA2, FADD2): half the issue slots for the argument and the row sum
+    float2 sum2a = make_float2(0.f, 0.f), sum2b = make_float2(0.f, 0.f);
+    const float2 sc2 = make_float2(sc, sc), nm2 = make_float2(-m_new, -m_new);
     uint32_t pk[32];
 #pragma unroll
-    for (int c = 0; c < 64; c += 2) {
-      const float e0 = ex2_approx(fmaf(x[c], sc, -m_new)), e1 = ex2_approx(fmaf(x[c + 1], sc, -m_new));
-      sum += e0 + e1;
-      pk[c >> 1] = pack_bf16x2(e0, e1);
+    for (int c = 0; c < 64; c += 4) {
+      const float2 t0 = ffma2(make_float2(x[c], x[c + 1]), sc2, nm2);
+      const float2 t1 = ffma2(make_float2(x[c + 2], x[c + 3]), sc2, nm2);
+      const float2 e0 = make_float2(ex2_approx(t0.x), ex2_approx(t0.y));
+      const float2 e1 = make_float2(ex2_approx(t1.x), ex2_approx(t1.y));
+      sum2a = fadd2(sum2a, e0);
+      sum2b = fadd2(sum2b, e1);
+      pk[c >> 1] = pack_bf16x2(e0.x, e0.y);
+      pk[(c >> 1) + 1] = pack_bf16x2(e1.x, e1.y);
     }
-    l = l * alpha + sum;
+    l = l * alpha + ((sum2a.x + sum2a.y) + (sum2b.x + sum2b.y));
     m = m_new;
 
     if (j > 0) {
@@ -256,21 +263,24 @@ __device__ __forceinline__ void softmax_m64(const Params& p, Ctl* ctl, uint8_t* 
       mB_new = mB;
     }
     const float alphaA = ex2_approx(mA - mA_new), alphaB = ex2_approx(mB - mB_new);
-    float sumA = 0.f, sumB = 0.f;
+    // packed fp32x2 FMA / ADD: half the issue slots of the scalar form for the argument and the sum
+    float2 sumA2 = make_float2(0.f, 0.f), sumB2 = make_float2(0.f, 0.f);
+    const float2 sc2 = make_float2(sc, sc);
+    const float2 nmA = make_float2(-mA_new, -mA_new), nmB = make_float2(-mB_new, -mB_new);
     uint32_t pa[8], pb[8];
 #pragma unroll
     for (int g = 0; g < 8; ++g) {
-      const float a0 = ex2_approx(fmaf(xa[2 * g], sc, -mA_new));
-      const float a1 = ex2_approx(fmaf(xa[2 * g + 1], sc, -mA_new));
-      const float b0 = ex2_approx(fmaf(xb[2 * g], sc, -mB_new));
-      const float b1 = ex2_approx(fmaf(xb[2 * g + 1], sc, -mB_new));
-      sumA += a0 + a1;
-      sumB += b0 + b1;
-      pa[g] = pack_bf16x2(a0, a1);
-      pb[g] = pack_bf16x2(b0, b1);
+      const float2 ta = ffma2(make_float2(xa[2 * g], xa[2 * g + 1]), sc2, nmA);
+      const float2 tb = ffma2(make_float2(xb[2 * g], xb[2 * g + 1]), sc2, nmB);
+      const float2 ea = make_float2(ex2_approx(ta.x), ex2_approx(ta.y));
+      const float2 eb = make_float2(ex2_approx(tb.x), ex2_approx(tb.y));
+      sumA2 = fadd2(sumA2, ea);
+      sumB2 = fadd2(sumB2, eb);
+      pa[g] = pack_bf16x2(ea.x, ea.y);
+      pb[g] = pack_bf16x2(eb.x, eb.y);
     }
-    lA = lA * alphaA + sumA;
-    lB = lB * alphaB + sumB;
+    lA = lA * alphaA + (sumA2.x + sumA2.y);
+    lB = lB * alphaB + (sumB2.x + sumB2.y);
     mA = mA_new;
     mB = mB_new;
 

@@ -40,6 +40,9 @@ __device__ __forceinline__ uint32_t bf2_max(uint32_t a, uint32_t b) {
   return r;
 }
 
+#ifndef BSA_POOL_TPS
+#define BSA_POOL_TPS 768
+#endif
 constexpr int kPasses = 8;  // key rows per thread: 8 x 16 B = 128 B in flight per thread
 
 // CTAs of BN*D/64 threads; thread (r0, c8) owns 8 adjacent columns of rows r0, r0 + RPP, ... of a
@@ -192,7 +195,7 @@ __device__ __forceinline__ void process_block(const PoolArgs<D, BN>& a, int w, c
 }
 
 template <int D, int BN>
-__global__ void __launch_bounds__(BN* D / 64, 768 / (BN * D / 64)) pool_kernel(const PoolArgs<D, BN> a) {
+__global__ void __launch_bounds__(BN* D / 64, BSA_POOL_TPS / (BN * D / 64)) pool_kernel(const PoolArgs<D, BN> a) {
   uint4 v[kPasses];
   load_block<D, BN>(a, static_cast<int>(blockIdx.x), v);
   process_block<D, BN>(a, static_cast<int>(blockIdx.x), v);
