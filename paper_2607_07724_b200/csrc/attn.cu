@@ -251,18 +251,21 @@ __device__ __forceinline__ void softmax_m64(const Params& p, Ctl* ctl, uint8_t* 
       mxA = fmax3(mxA, xa[c], xa[c + 1]);
       mxB = fmax3(mxB, xb[c], xb[c + 1]);
     }
-    mxA = fmaxf(mxA, __shfl_xor_sync(0xffffffffu, mxA, 1));
-    mxB = fmaxf(mxB, __shfl_xor_sync(0xffffffffu, mxB, 1));
-    mxA = fmaxf(mxA, __shfl_xor_sync(0xffffffffu, mxA, 2));
-    mxB = fmaxf(mxB, __shfl_xor_sync(0xffffffffu, mxB, 2));
-    float mA_new = fmaxf(mA, mxA * sc), mB_new = fmaxf(mB, mxB * sc);
-    // lazy rescale: keep the stale reference maxima unless some row of this warp grew by > 2^8
-    const bool any = __any_sync(0xffffffffu, (mA_new - mA > 8.0f) || (mB_new - mB > 8.0f));
-    if (!any) {
-      mA_new = mA;
-      mB_new = mB;
+    // lazy rescale: keep the stale reference maxima unless some row of this warp grew by > 2^8.
+    // The test only needs each thread's partial maximum (a row exceeds iff one of its four threads
+    // does), so the quad shuffles and the alphas are off the common path.
+    const bool any = __any_sync(0xffffffffu, (fmaf(mxA, sc, -mA) > 8.0f) || (fmaf(mxB, sc, -mB) > 8.0f));
+    float mA_new = mA, mB_new = mB, alphaA = 1.0f, alphaB = 1.0f;
+    if (any) {
+      mxA = fmaxf(mxA, __shfl_xor_sync(0xffffffffu, mxA, 1));
+      mxB = fmaxf(mxB, __shfl_xor_sync(0xffffffffu, mxB, 1));
+      mxA = fmaxf(mxA, __shfl_xor_sync(0xffffffffu, mxA, 2));
+      mxB = fmaxf(mxB, __shfl_xor_sync(0xffffffffu, mxB, 2));
+      mA_new = fmaxf(mA, mxA * sc);
+      mB_new = fmaxf(mB, mxB * sc);
+      alphaA = ex2_approx(mA - mA_new);
+      alphaB = ex2_approx(mB - mB_new);
     }
-    const float alphaA = ex2_approx(mA - mA_new), alphaB = ex2_approx(mB - mB_new);
     // packed fp32x2 FMA / ADD: half the issue slots of the scalar form for the argument and the sum
     float2 sumA2 = make_float2(0.f, 0.f), sumB2 = make_float2(0.f, 0.f);
     const float2 sc2 = make_float2(sc, sc);
