@@ -145,7 +145,9 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   if (warp == 4) {
     // ---- TMA producer ------------------------------------------------------------------------
     if (lane == 0) {
-      int li = 0, ring = 0;
+      const int stages = p.stages;
+      int li = 0, s = 0;
+      uint32_t ph = 0;
       for (int w = w0; w < p.n_items; w += wstep, ++li) {
         const Item im = decode_item<C::NH>(p, w);
         if (li > 0) mbar_wait(smem_u32(&ctl->b_free), (li - 1) & 1);   // MMAs of the previous item done
@@ -159,23 +161,35 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             tma_prefetch_5d(&tmQ, 0, nx.t * BN, c64, nx.h0, nx.b);
         }
         for (int c = 0; c < im.n_chunks; ++c) {
-          for (int kc = 0; kc < C::KCHUNKS; ++kc, ++ring) {
-            const int s = ring % p.stages;
+#pragma unroll
+          for (int kc = 0; kc < C::KCHUNKS; ++kc) {
             const int pa = kc / C::DC, c64 = kc % C::DC;
             const int mem_plane = QUEST ? (1 - pa) : pa;   // memory order: [kmin, kmax] / [hi, mid, lo]
-            mbar_wait(smem_u32(&ctl->a_empty[s]), ((ring / p.stages) & 1) ^ 1);
+            mbar_wait(smem_u32(&ctl->a_empty[s]), ph ^ 1u);
             mbar_arrive_expect_tx(smem_u32(&ctl->a_full[s]), kAStageBytes);
             tma_load_5d(smem_u32(a_s + s * kAStageBytes), &tmA, smem_u32(&ctl->a_full[s]), c64 * 64,
                         c * kABlocks, im.g, im.b, mem_plane);
+            if (++s == stages) {
+              s = 0;
+              ph ^= 1u;
+            }
           }
         }
       }
     }
   } else if (warp == 5) {
     // ---- MMA issuer --------------------------------------------------------------------------
+    // One thread; it must stay cheap: an ncu source view of the first persistent version showed this
+    // thread executing ~700 scalar instructions per 16-MMA chunk (runtime `ring % stages`, descriptor
+    // rebuilds), i.e. longer than the MMAs it issues, with the tensor pipe 50 % idle.  The ring slot
+    // and phase are tracked incrementally and the descriptors are a base plus a small constant.
     if (lane == 0) {
       const uint32_t b_a = smem_u32(b_s), a_a = smem_u32(a_s);
-      int li = 0, ring = 0, cg = 0;
+      const uint64_t adesc0 = umma_smem_desc(a_a, 16, 1024);
+      const uint64_t bdesc0 = umma_smem_desc(b_a, 16, 1024);
+      const int stages = p.stages;
+      int li = 0, cg = 0, s = 0;
+      uint32_t ph = 0;
       for (int w = w0; w < p.n_items; w += wstep, ++li) {
         const Item im = decode_item<C::NH>(p, w);
         const uint32_t idesc = umma_idesc_bf16(kABlocks, im.nh * BN, 0, 0);
@@ -188,18 +202,21 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             tc_fence_after();
           }
           const uint32_t tD = tmem + buf * C::NROWS;
-          for (int kc = 0; kc < C::KCHUNKS; ++kc, ++ring) {
-            const int s = ring % p.stages;
-            const int bchunk = QUEST ? kc : (kc % C::DC);
-            mbar_wait(smem_u32(&ctl->a_full[s]), (ring / p.stages) & 1);
-            tc_fence_after();
 #pragma unroll
-            for (int ks = 0; ks < 4; ++ks) {
-              const uint64_t ad = umma_smem_desc(a_a + s * kAStageBytes + ks * 32, 16, 1024);
-              const uint64_t bd = umma_smem_desc(b_a + bchunk * C::B_CHUNK_BYTES + ks * 32, 16, 1024);
-              umma_ss(tD, ad, bd, idesc, (kc > 0) || (ks > 0));
-            }
+          for (int kc = 0; kc < C::KCHUNKS; ++kc) {
+            const int bchunk = QUEST ? kc : (kc % C::DC);
+            mbar_wait(smem_u32(&ctl->a_full[s]), ph);
+            tc_fence_after();
+            const uint64_t ad = adesc0 + static_cast<uint64_t>((s * kAStageBytes) >> 4);
+            const uint64_t bd = bdesc0 + static_cast<uint64_t>((bchunk * C::B_CHUNK_BYTES) >> 4);
+#pragma unroll
+            for (int ks = 0; ks < 4; ++ks)
+              umma_ss(tD, ad + 2 * ks, bd + 2 * ks, idesc, (kc > 0) || (ks > 0));   // +32 B per K step
             tc_commit(smem_u32(&ctl->a_empty[s]));
+            if (++s == stages) {
+              s = 0;
+              ph ^= 1u;
+            }
           }
           tc_commit(smem_u32(&ctl->acc_full[buf]));
         }
@@ -313,6 +330,9 @@ bsa_status run_score_tc(const Dims& S, const void* Q, const char* meta, const Me
     return fail(BSA_ERR_UNSUPPORTED, "select: %d blocks per sequence need too much shared memory", S.NB);
   int stages = static_cast<int>((budget - fixed) / kAStageBytes);
   p.stages = stages > kMaxStages ? kMaxStages : stages;
+#ifdef BSA_TC_STAGE_CAP
+  if (p.stages > BSA_TC_STAGE_CAP) p.stages = BSA_TC_STAGE_CAP;
+#endif
   const size_t smem = fixed + static_cast<size_t>(p.stages) * kAStageBytes;
 
   CUtensorMap tq, ta;
