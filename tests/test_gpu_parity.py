@@ -215,6 +215,34 @@ def test_sparse_attention_is_deterministic(bsa, name, policy, reps):
             assert torch.equal(lse, first[1]), f"launch {i}: lse differs"
 
 
+def test_select_and_dense_are_deterministic(bsa):
+    """Same guard for the selection pipeline (all outputs) and the dense kernel at C2."""
+    import torch
+    cfg, inp, _ = _case("C2")
+    Q, K, V = _dev(inp)
+    buf = bsa.bsa_build_block_meta(K, cfg.block, 3)
+    first = None
+    for policy in ("router_quest", "router"):
+        first = None
+        for i in range(8):
+            r = bsa.bsa_select(Q, buf, K, cfg.block, policy, cfg.k_budget, 0.25)
+            torch.cuda.synchronize()
+            cur = {k: r[k].clone() for k in ("kv_idx", "kv_count", "sigma", "sigma_bar", "trigger", "tau")}
+            if first is None:
+                first = cur
+            else:
+                for k in cur:
+                    assert torch.equal(cur[k].view(torch.uint8), first[k].view(torch.uint8)), f"{policy} launch {i}: {k}"
+    O0 = None
+    for i in range(6):
+        O, _ = bsa.bsa_dense_attn_fwd(Q, K, V, cfg.block)
+        torch.cuda.synchronize()
+        if O0 is None:
+            O0 = O.clone()
+        else:
+            assert torch.equal(O.view(torch.int16), O0.view(torch.int16)), f"dense launch {i}"
+
+
 def test_sparse_attention_edge_cases(bsa):
     """permuted rows, sentinel / future entries skipped, kv_count = NULL, empty rows -> zeros,
     k_budget >= N_B reduces to dense."""
