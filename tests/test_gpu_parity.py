@@ -243,6 +243,48 @@ def test_select_and_dense_are_deterministic(bsa):
             assert torch.equal(O.view(torch.int16), O0.view(torch.int16)), f"dense launch {i}"
 
 
+# ---- every (block, head_dim) pair the C ABI accepts, not only the ones the five configs use ----------
+@pytest.mark.parametrize("block,d", [(64, 64), (64, 128), (64, 256), (128, 64), (128, 128), (128, 256)])
+@pytest.mark.parametrize("policy", ["router", "router_quest"])
+def test_all_block_headdim_pairs(bsa, block, d, policy):
+    """pool -> select -> sparse attention and the dense kernel for each supported (block, head_dim);
+    GQA 6/2, ragged tile count (9 tiles), k_budget 4, i.i.d. inputs of the C1 recipe."""
+    import dataclasses
+    import torch
+    key = f"pair{block}x{d}"
+    if key not in _CACHE:
+        cfg = dataclasses.replace(synth.CONFIGS["C1"], name=key, number=60 + block // 64 + d // 64 * 3,
+                                  seqlen=9 * block, n_q_heads=6, n_kv_heads=2, head_dim=d, block=block)
+        inp = synth.make_inputs(cfg)
+        _CACHE[key] = (cfg, inp, oracle.pool(inp.K, block))
+    cfg, inp, meta_np = _CACHE[key]
+    Q, K, V = _dev(inp)
+    buf = bsa.bsa_build_block_meta(K, block, 3)
+    kmean, kmin, kmax = bsa.meta_views(buf, K.shape, block)
+    assert np.array_equal(kmean[0].cpu().numpy().view(np.uint32), meta_np[0].view(np.uint32))
+    assert np.array_equal(bf16_to_f32(bf16_bits(kmin[0])), bf16_to_f32(meta_np[1]))
+    assert np.array_equal(bf16_to_f32(bf16_bits(kmax[0])), bf16_to_f32(meta_np[2]))
+    r = bsa.bsa_select(Q, buf, K, block, policy, cfg.k_budget, 0.25)
+    O, lse = bsa.bsa_sparse_attn_fwd(Q, K, V, r["kv_idx"], r["kv_count"], block, want_lse=True)
+    Od, _ = bsa.bsa_dense_attn_fwd(Q, K, V, block)
+    torch.cuda.synchronize()
+    orc = oracle.select(inp.Q, meta_np, block, policy, cfg.k_budget, 0.25, want_scores=True)
+    log = []
+    compare_select(_gpu_select_np(r), orc, cfg.n_blocks, cfg.k_budget, log)
+    tied = {(e[1], e[2]) for e in log if e[0] == "kv_idx"}
+    flipped_t = {e[1] for e in log if e[0] == "trigger"}
+    T, H = cfg.n_blocks, cfg.n_q_heads
+    pairs = [(t, h) for h in range(H) for t in range(T) if (h, t) not in tied and t not in flipped_t]
+    ref, ref_lse = oracle.attn_pairs(inp.Q, inp.K, inp.V, block, pairs, orc["kv_idx"], orc["kv_count"])
+    Og = O[0].float().cpu().numpy().reshape(H, T, block, d)
+    compare_attn(np.stack([Og[h, t] for t, h in pairs]), ref, f"pair {block}x{d} sparse")
+    got_lse = lse[0].cpu().numpy().reshape(H, T, block)
+    np.testing.assert_allclose(np.stack([got_lse[h, t] for t, h in pairs]), ref_lse, rtol=0, atol=2e-3)
+    allp = [(t, h) for h in range(H) for t in range(T)]
+    refd, _ = oracle.attn_pairs(inp.Q, inp.K, inp.V, block, allp)
+    compare_attn(Od[0].float().cpu().numpy().reshape(H * T, block, d), refd, f"pair {block}x{d} dense")
+
+
 def test_sparse_attention_edge_cases(bsa):
     """permuted rows, sentinel / future entries skipped, kv_count = NULL, empty rows -> zeros,
     k_budget >= N_B reduces to dense."""
