@@ -43,6 +43,22 @@ __device__ __forceinline__ uint32_t bf2_max(uint32_t a, uint32_t b) {
 #ifndef BSA_POOL_TPS
 #define BSA_POOL_TPS 768
 #endif
+// packed fp32x2 adds with directed rounding (FADD2.RP / FADD2.RM): one issue slot for both halves of a word
+__device__ __forceinline__ float2 fadd2_ru(float2 a, float2 b) {
+  float2 d;
+  asm("{\n\t.reg .b64 ra, rb, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\t"
+      "add.rp.f32x2 rd, ra, rb;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+      : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+  return d;
+}
+__device__ __forceinline__ float2 fadd2_rd(float2 a, float2 b) {
+  float2 d;
+  asm("{\n\t.reg .b64 ra, rb, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\t"
+      "add.rm.f32x2 rd, ra, rb;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+      : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+  return d;
+}
+
 constexpr int kPasses = 8;  // key rows per thread: 8 x 16 B = 128 B in flight per thread
 
 // CTAs of BN*D/64 threads; thread (r0, c8) owns 8 adjacent columns of rows r0, r0 + RPP, ... of a
@@ -110,11 +126,13 @@ __device__ __forceinline__ void process_block(const PoolArgs<D, BN>& a, int w, c
     const uint32_t w[4] = {v[p].x, v[p].y, v[p].z, v[p].w};
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-      const float lo = bf_lo(w[i]), hv = bf_hi(w[i]);
-      ru[2 * i] = __fadd_ru(ru[2 * i], lo);
-      rd[2 * i] = __fadd_rd(rd[2 * i], lo);
-      ru[2 * i + 1] = __fadd_ru(ru[2 * i + 1], hv);
-      rd[2 * i + 1] = __fadd_rd(rd[2 * i + 1], hv);
+      const float2 x = make_float2(bf_lo(w[i]), bf_hi(w[i]));
+      const float2 u = fadd2_ru(make_float2(ru[2 * i], ru[2 * i + 1]), x);
+      const float2 dn = fadd2_rd(make_float2(rd[2 * i], rd[2 * i + 1]), x);
+      ru[2 * i] = u.x;
+      ru[2 * i + 1] = u.y;
+      rd[2 * i] = dn.x;
+      rd[2 * i + 1] = dn.y;
       mn2[i] = bf2_min(mn2[i], w[i]);
       mx2[i] = bf2_max(mx2[i], w[i]);
     }
