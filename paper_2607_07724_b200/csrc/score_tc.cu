@@ -260,7 +260,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         const int blk = c * kABlocks + warp * 32 + lane;
         const uint32_t tD = tmem + lane_base + buf * C::NROWS;
         for (int j = 0; j < im.nh; ++j) {
-          float mx = -INFINITY;
+          float m0 = -INFINITY, m1 = -INFINITY, m2 = -INFINITY, m3 = -INFINITY;   // four independent chains
 #pragma unroll
           for (int c0 = 0; c0 < BN; c0 += 64) {
             uint32_t ra[32], rb[32];
@@ -268,9 +268,14 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             tmem_ld32(tD + j * BN + c0 + 32, rb);
             tmem_ld_wait();
 #pragma unroll
-            for (int i = 0; i < 32; ++i)
-              mx = fmax3(mx, __uint_as_float(ra[i]), __uint_as_float(rb[i]));
+            for (int i = 0; i < 32; i += 4) {
+              m0 = fmax3(m0, __uint_as_float(ra[i]), __uint_as_float(rb[i]));
+              m1 = fmax3(m1, __uint_as_float(ra[i + 1]), __uint_as_float(rb[i + 1]));
+              m2 = fmax3(m2, __uint_as_float(ra[i + 2]), __uint_as_float(rb[i + 2]));
+              m3 = fmax3(m3, __uint_as_float(ra[i + 3]), __uint_as_float(rb[i + 3]));
+            }
           }
+          const float mx = fmaxf(fmax3(m0, m1, m2), m3);
           if (blk <= im.t) sc[j * p.nbpad + blk] = okey(QUEST ? mx : mx * p.inv_sqrt_d);   // Eq.3 (G8)
         }
         tc_fence_before();
