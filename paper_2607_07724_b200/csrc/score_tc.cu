@@ -183,7 +183,8 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     // thread executing ~700 scalar instructions per 16-MMA chunk (runtime `ring % stages`, descriptor
     // rebuilds), i.e. longer than the MMAs it issues, with the tensor pipe 50 % idle.  The ring slot
     // and phase are tracked incrementally and the descriptors are a base plus a small constant.
-    if (lane == 0) {
+    {   // the whole warp runs the loop (warp-uniform addresses and descriptors); one lane issues
+      const bool leader = elect_one();
       const uint32_t b_a = smem_u32(b_s), a_a = smem_u32(a_s);
       const uint64_t adesc0 = umma_smem_desc(a_a, 16, 1024);
       const uint64_t bdesc0 = umma_smem_desc(b_a, 16, 1024);
@@ -211,16 +212,17 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             const uint64_t bd = bdesc0 + static_cast<uint64_t>((bchunk * C::B_CHUNK_BYTES) >> 4);
 #pragma unroll
             for (int ks = 0; ks < 4; ++ks)
-              umma_ss(tD, ad + 2 * ks, bd + 2 * ks, idesc, (kc > 0) || (ks > 0));   // +32 B per K step
-            tc_commit(smem_u32(&ctl->a_empty[s]));
+              if (leader) umma_ss(tD, ad + 2 * ks, bd + 2 * ks, idesc, (kc > 0) || (ks > 0));   // +32 B per K step
+            if (leader) tc_commit(smem_u32(&ctl->a_empty[s]));
+            __syncwarp();
             if (++s == stages) {
               s = 0;
               ph ^= 1u;
             }
           }
-          tc_commit(smem_u32(&ctl->acc_full[buf]));
+          if (leader) tc_commit(smem_u32(&ctl->acc_full[buf]));
         }
-        tc_commit(smem_u32(&ctl->b_free));   // every MMA that reads this item's B planes has completed
+        if (leader) tc_commit(smem_u32(&ctl->b_free));   // every MMA that reads this item's B planes has completed
       }
     }
   } else if (warp < 4) {
