@@ -1,23 +1,31 @@
 #!/usr/bin/env python
 """bench.py -- one JSON line for the selection + sparse-attention prefill path.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2|C3a|C3b|C4|C5|C1]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3b|C2|C3a|C3c|C4|C5|C1]
                     [--policy router_quest] [--q-frac 0.25] [--no-extra] [--impl reference]
 
 A step is one pass of the whole hot path over one synthetic prefill layer:
 bsa_build_block_meta -> bsa_select -> bsa_sparse_attn_fwd (rows 1-6, the "sparse prefill attention")
 and bsa_dense_attn_fwd (row 7, the "x dense" denominator).  Each stage is bracketed by CUDA events on
 the launching stream; L2 is flushed (512 MiB memset) before every step, outside the event pairs.
+Default workload: C3b, the 128K Qwen2.5-7B-shaped layer with router_quest that BASELINE.json's
+north_star names as the headline ("router_quest sparse prefill at 128K ... as a measured ratio of this
+library's own dense kernel time").
 
   value        = ms of rows 1-6 (pool + select + sparse attention), mean over the K timed steps,
-                 inputs resident in HBM
+                 inputs resident in HBM; `stats` carries median and min per stage
   ms_per_step  = rows 1-7 (value + dense kernel)
-  x_dense      = value / dense ms (the paper's "x dense wall time", attention only)
+  x_dense      = value / dense ms (the paper's "x dense wall time", attention only), phases timed apart,
+                 each with its own clock record; x_dense_interleaved = the same ratio with the dense
+                 kernel launched directly before every sparse pass (the other ordering)
   e2e          = the same rows 1-6 through the C ABI from pinned HOST buffers: H2D of Q, K, V and D2H of
                  O inside the timed region
   roofline     = the sparse attention kernel (dominant kernel of rows 1-6) against the measured bf16 peak
-  cpu_baseline = the CPU oracle (oracle/), timed on this host's cores on a stratified 1/16 sample of the
-                 (tile, head) problems of the same workload, scaled to the full workload
+  cpu_baseline = the CPU oracle (oracle/), timed on this host's cores on a bounded sample of the same
+                 workload; `measured_ms` is what was timed, `scale` the factor to the full workload,
+                 `value` their product, labelled `extrapolated`
+  extra        = the other BASELINE.json configs (C2, C3a, C4, C5, C3c) and the k_budget / q sweeps the
+                 paper itself varies, fewer steps each
 
 N > 1: the path does not shard (replicas only); every rank runs an independent
 replica, the time is the max over ranks.
@@ -124,24 +132,45 @@ def ncu_traffic(key: str):
 
 
 # ---- the CPU oracle legs --------------------------------------------------------------------------
+def golden_route(cfg, policy: str, q_frac: float):
+    """(tau, trigger[T]) of the WHOLE sequence from the oracle-written golden (tests/golden/), or None."""
+    case = f"{cfg.name}/{policy}"
+    p = os.path.join(ROOT, "tests", "golden", "routing_" + case.replace("/", "_") + ".json")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        d = json.load(f)
+    r = d["routes"].get(repr(float(q_frac)))
+    if r is None or d["seed"] != cfg.seed or d["seqlen"] != cfg.seqlen:
+        return None
+    return float(r["tau"]), np.frombuffer(r["trigger_bits"].encode(), dtype=np.uint8) - ord("0")
+
+
 def oracle_sample_ms(cfg, inp, policy: str, q_frac: float, stride: int = 16):
-    """Oracle rows 1-6 on a stratified 1/stride sample of tiles (all heads), scaled by `stride`.
-    Pooling is run in full.  Returns (ms scaled to the full workload, seconds of CPU work, sample text)."""
+    """Oracle rows 1-6.  stride == 1: the whole workload, with the oracle's own routing.  stride > 1: a
+    stratified sample of tiles (every stride-th, all heads); pooling runs in full; the trigger of the
+    sampled tiles comes from the oracle's full-sequence routing (tests/golden/routing_*.json, written
+    by oracle/ alone) when that file exists, else from the sample's own quantile (said in the text).
+    Returns dict(measured_ms, scale, value, seconds, sample)."""
     import oracle
     oracle.max_threads()                       # builds / loads the oracle library outside the timed part
-    T, H = cfg.n_blocks, cfg.n_q_heads
-    stride = min(stride, max(T // 2, 1))
+    T, H, k = cfg.n_blocks, cfg.n_q_heads, cfg.k_budget
+    stride = max(1, min(stride, max(T // 2, 1)))
     tiles = np.arange(stride // 2, T, stride)
+    n = len(tiles)
+    router = policy in ("router", "router_quest")
+    gold = golden_route(cfg, policy, q_frac) if (stride > 1 and router) else None
     t0 = time.perf_counter()
     meta = oracle.pool(inp.K, cfg.block)
     t1 = time.perf_counter()
-    r = oracle.select_tiles(inp.Q, meta, cfg.block, policy, cfg.k_budget, tiles)
-    # routing of the sampled tiles (the threshold needs every tile; on the sample it is the sample's own
-    # quantile, which keeps the triggered fraction -- and therefore the attention work -- representative)
-    sigma_bar, tau, trig = oracle.route(r["sigma"], policy, q_frac)
-    W = oracle.kv_width(policy, cfg.k_budget)
-    k = cfg.k_budget
-    n = len(tiles)
+    r = oracle.select_tiles(inp.Q, meta, cfg.block, policy, k, tiles)
+    if gold is not None:
+        trig = gold[1][tiles]
+        how = "trigger of the sampled tiles from the oracle's full-sequence routing (tests/golden)"
+    else:
+        _, _, trig = oracle.route(r["sigma"], policy, q_frac)
+        how = "oracle routing" if stride == 1 else "routing by the sample's own quantile"
+    W = oracle.kv_width(policy, k)
     kv_idx = np.full((H, T, W), T, np.int32)
     kv_count = np.zeros((H, T), np.int32)
     for i, t in enumerate(tiles):
@@ -152,14 +181,30 @@ def oracle_sample_ms(cfg, inp, policy: str, q_frac: float, stride: int = 16):
     pairs = [(int(t), h) for t in tiles for h in range(H)]
     oracle.attn_pairs(inp.Q, inp.K, inp.V, cfg.block, pairs, kv_idx, kv_count, want_lse=False)
     t3 = time.perf_counter()
-    scaled = (t1 - t0) + (t3 - t1) * (T / n)
-    text = (f"pooling in full; scoring+top-k+sigma+routing+fill and sparse attention on {n} of {T} tiles "
-            f"(every {stride}th, all {H} heads), time scaled by {T / n:.3g}")
-    return scaled * 1e3, (t3 - t0), text
+    pool_ms, rest_ms = (t1 - t0) * 1e3, (t3 - t1) * 1e3
+    scale = T / n
+    if stride == 1:
+        text = f"the whole workload: all {T} tiles x {H} heads, {how}"
+    else:
+        text = (f"pooling in full ({pool_ms:.0f} ms); scoring + top-k + sigma + fill + sparse attention on "
+                f"{n} of {T} tiles (every {stride}th, all {H} heads; {rest_ms:.0f} ms measured, x{scale:.4g}); {how}")
+    return {"measured_ms": pool_ms + rest_ms, "scale": scale, "value": pool_ms + rest_ms * scale,
+            "extrapolated": stride > 1, "seconds": t3 - t0, "sample": text}
+
+
+def reference_stride(cfg, steps_total: int, cores: int) -> int:
+    """Tile stride (a power of two) that keeps the whole reference run near 2-3 minutes: the oracle does
+    about 1.2e8 MAC/s per core (measured: C2 in full, 6e10 scoring + 7e10 attention MAC, 34 s on 16)."""
+    work = cfg.n_blocks * (cfg.n_blocks + 1) / 2 * cfg.block * cfg.head_dim * cfg.n_q_heads * 4.0
+    per_step_s = 150.0 / max(steps_total, 1)
+    need = work / (1.2e8 * max(cores, 1) * per_step_s)
+    return int(min(512, max(1, 2 ** math.ceil(math.log2(max(need, 1))))))
 
 
 def run_reference(args):
-    """--impl reference: the CPU oracle as it stands, on the host cores, same config / metric."""
+    """--impl reference: the CPU oracle as it stands, on the host cores, same config / metric.  Each step
+    is a bounded sample of the workload; `ms_per_step` is what a step really took, `value` the same metric
+    as the GPU arm (ms for the full workload) = pooling + measured rest x scale, labelled extrapolated."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
@@ -168,23 +213,27 @@ def run_reference(args):
     cfg = synth.CONFIGS[args.workload]
     inp = synth.make_inputs(cfg)
     oracle.build()
-    stride = 64 if cfg.seqlen >= 32768 else 4          # keeps warmup+steps within a few minutes
-    times = []
+    stride = reference_stride(cfg, args.warmup + args.steps, oracle.max_threads())
+    runs = []
     for i in range(args.warmup + args.steps):
-        ms, _, text = oracle_sample_ms(cfg, inp, args.policy, args.q_frac, stride)
+        r = oracle_sample_ms(cfg, inp, args.policy, args.q_frac, stride)
         if i >= args.warmup:
-            times.append(ms)
-    v = float(np.mean(times))
+            runs.append(r)
+    v = float(np.mean([r["value"] for r in runs]))
+    measured = float(np.mean([r["measured_ms"] for r in runs]))
+    base = {"kind": "oracle", "cores": oracle.max_threads(), "sample": runs[-1]["sample"],
+            "measured_ms": measured, "scale": runs[-1]["scale"], "extrapolated": runs[-1]["extrapolated"]}
     line = {
         "impl": "reference", "metric": METRIC, "value": v, "unit": "ms", "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": v, "higher_is_better": False,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": measured, "higher_is_better": False,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64 accumulate, f32 results (CPU oracle)",
         "data": "synthetic",
         "config": workload_config(cfg, args),
-        "cpu_baseline": {"value": v, "unit": "ms", "cores": oracle.max_threads(), "kind": "oracle",
-                         "sample": text},
+        "cpu_baseline": dict(base, value=v, unit="ms"),
         "e2e": {"value": v, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
+        "note": "value = ms for the full workload (extrapolated from the sample when scale > 1); "
+                "ms_per_step = the measured time of one step of this arm",
     }
     print(json.dumps(line), flush=True)
 
@@ -193,7 +242,8 @@ def workload_config(cfg, args):
     return {"workload": f"{cfg.name}: B1 N={cfg.seqlen} Hq={cfg.n_q_heads} Hkv={cfg.n_kv_heads} "
                         f"d={cfg.head_dim} block={cfg.block} k_budget={cfg.k_budget}",
             "policy": args.policy, "q_frac": args.q_frac, "k_budget": cfg.k_budget, "seqlen": cfg.seqlen,
-            "order": "K timed passes of rows 1-6, then K timed passes of row 7 (dense reference kernel)",
+            "order": "K timed passes of rows 1-6, then K timed passes of row 7 (dense reference kernel), then 3 "
+                     "interleaved passes (dense, sparse) for x_dense_interleaved",
             "l2": "flushed before every step (512 MiB memset outside the event pairs); "
                   "Q+K+V+O also exceed the 126 MB L2",
             "parallelism": "replicas only"}
@@ -271,46 +321,78 @@ class Runner:
             e.record()
             ev.append(e)
 
-    def timed_steps(self, steps, warmup, with_dense=True):
-        """Returns per-stage mean ms over `steps` steps: pool, select, sparse, dense.
+    def timed_steps(self, steps, warmup, with_dense=True, clocks_index=None, interleaved=0):
+        """Per-stage ms lists over `steps` steps: pool, select, sparse, dense (+ clock records per phase).
 
         The K timed steps run as K passes of rows 1-6 followed by K passes of row 7 (the dense
         kernel): a dense launch (full tensor-pipe power for 7-115 ms) directly in front of the sparse
         path drops the SM clock from 1965 to ~1665 MHz for the next kernels and inflates the sparse
-        attention by 10-25 % (measured: 1.81 -> 2.13 ms at C2), which is an artefact of interleaving
-        the reference kernel, not a property of the sparse path."""
+        attention by 10-25 % (measured: 1.81 -> 2.13 ms at C2).  Both phases get their own clock
+        record, and `interleaved` > 0 adds that many steps in the other ordering (dense, then sparse,
+        back to back) so that both bounds of the ratio are on the line."""
         torch = self.torch
+
+        def ev():
+            e = torch.cuda.Event(enable_timing=True)
+            e.record()
+            return e
+
         for _ in range(warmup):
             self.flush_l2()
             self.sparse_path()
-        if with_dense:
-            for _ in range(warmup):
-                self.flush_l2()
-                self.dense()
         torch.cuda.synchronize()
-        all_ev, dense_ev = [], []
+        clk = {}
+        sampler = ClockSampler(clocks_index) if clocks_index is not None else None
+        if sampler:
+            sampler.start()
+        all_ev, dense_ev, inter_ev = [], [], []
         for _ in range(steps):
             self.flush_l2()
-            ev = []
-            self.sparse_path(ev=ev)
-            all_ev.append(ev)
+            evs = []
+            self.sparse_path(ev=evs)
+            all_ev.append(evs)
+        torch.cuda.synchronize()
+        if sampler:
+            clk["sparse_phase"] = sampler.stop()
         if with_dense:
+            for _ in range(min(warmup, 3)):
+                self.flush_l2()
+                self.dense()
+            torch.cuda.synchronize()
+            sampler = ClockSampler(clocks_index) if clocks_index is not None else None
+            if sampler:
+                sampler.start()
             for _ in range(steps):
                 self.flush_l2()
-                e0 = torch.cuda.Event(enable_timing=True)
-                e0.record()
-                ev = [e0]
-                self.dense(ev=ev)
-                dense_ev.append(ev)
-        torch.cuda.synchronize()
+                e0 = ev()
+                self.dense()
+                dense_ev.append((e0, ev()))
+            torch.cuda.synchronize()
+            if sampler:
+                clk["dense_phase"] = sampler.stop()
+            for _ in range(interleaved):
+                self.flush_l2()
+                e0 = ev()
+                self.dense()
+                e1 = ev()
+                self.flush_l2()
+                evs = []
+                self.sparse_path(ev=evs)
+                inter_ev.append((e0, e1, evs))
+            torch.cuda.synchronize()
         names = ["pool", "select", "sparse"]
         per = {n: [] for n in names}
-        for ev in all_ev:
+        for evs in all_ev:
             for i, n in enumerate(names):
-                per[n].append(ev[i].elapsed_time(ev[i + 1]))
+                per[n].append(evs[i].elapsed_time(evs[i + 1]))
+        per["path"] = [evs[0].elapsed_time(evs[3]) for evs in all_ev]      # rows 1-6 incl. launch gaps
         if with_dense:
-            per["dense"] = [ev[0].elapsed_time(ev[1]) for ev in dense_ev]
-        return {n: float(np.mean(v)) for n, v in per.items()}, {n: float(np.min(v)) for n, v in per.items()}
+            per["dense"] = [a.elapsed_time(b) for a, b in dense_ev]
+            if inter_ev:
+                per["dense_interleaved"] = [a.elapsed_time(b) for a, b, _ in inter_ev]
+                per["path_interleaved"] = [evs[0].elapsed_time(evs[3]) for _, _, evs in inter_ev]
+        self.clocks = clk
+        return per
 
     def e2e_steps(self, steps, warmup):
         """rows 1-6 from pinned host buffers: H2D Q,K,V + kernels + D2H O inside the timed region."""
@@ -332,6 +414,37 @@ class Runner:
         h2d = sum(x.numel() * 2 for x in (self.hQ, self.hK, self.hV))
         d2h = self.hO.numel() * 2
         return float(np.mean(times)), h2d, d2h
+
+
+def stats_of(per: dict) -> dict:
+    """mean / median / min per stage (SURVEY 8(d) "Timing procedure": >= 8 repetitions, median and min)."""
+    return {n: {"mean": float(np.mean(v)), "median": float(np.median(v)), "min": float(np.min(v)), "n": len(v)}
+            for n, v in per.items()}
+
+
+def summarize(cfg, per: dict, kv_sum: int, peaks: dict) -> dict:
+    """Per-config record: stage ms (mean), x dense, tokens/s, roofline fractions."""
+    st = stats_of(per)
+    m = {n: st[n]["mean"] for n in st}
+    alg = algorithmic(cfg, kv_sum)
+    path = m["pool"] + m["select"] + m["sparse"]
+    peak_tf = peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"])
+    rec = {"seqlen": cfg.seqlen, "sparse_path_ms": path, "pool_ms": m["pool"], "select_ms": m["select"],
+           "sparse_attn_ms": m["sparse"], "stats": st, "kv_count_sum": kv_sum,
+           "mean_blocks_per_tile": kv_sum / (cfg.n_q_heads * cfg.n_blocks),
+           "tokens_per_s": cfg.seqlen / (path * 1e-3),
+           "pool_gbs": alg["pool_bytes"] / (m["pool"] * 1e-3) / 1e9,
+           "pool_frac_of_hbm_peak": alg["pool_bytes"] / (m["pool"] * 1e-3) / 1e9 / peaks["hbm_gbs"],
+           "sparse_tflops": alg["sparse_flops"] / (m["sparse"] * 1e-3) / 1e12,
+           "sparse_frac_of_bf16_peak": alg["sparse_flops"] / (m["sparse"] * 1e-3) / 1e12 / peak_tf}
+    if "dense" in m:
+        rec.update({"dense_attn_ms": m["dense"], "x_dense": path / m["dense"],
+                    "x_dense_kernel_only": m["sparse"] / m["dense"],
+                    "dense_tflops": alg["dense_flops"] / (m["dense"] * 1e-3) / 1e12,
+                    "dense_frac_of_bf16_peak": alg["dense_flops"] / (m["dense"] * 1e-3) / 1e12 / peak_tf})
+    if "dense_interleaved" in m:
+        rec["x_dense_interleaved"] = m["path_interleaved"] / m["dense_interleaved"]
+    return rec
 
 
 def run_gpu(args):
@@ -364,11 +477,13 @@ def run_gpu(args):
     barrier()
     clocks.start()
     t_wall0 = time.perf_counter()
-    mean, best = run.timed_steps(args.steps, args.warmup)
+    per = run.timed_steps(args.steps, args.warmup, clocks_index=local, interleaved=min(3, args.steps))
     barrier()
     wall_ms = (time.perf_counter() - t_wall0) * 1e3
     clk = clocks.stop()
+    clk["phases"] = run.clocks
 
+    mean = {n: float(np.mean(v)) for n, v in per.items()}
     sparse_ms = mean["pool"] + mean["select"] + mean["sparse"]
     step_ms = sparse_ms + mean["dense"]
     sparse_ms, step_ms = max_over_ranks([sparse_ms, step_ms], world, "cuda")
@@ -383,12 +498,13 @@ def run_gpu(args):
             dist.destroy_process_group()
         return
 
-    tf_sparse = alg["sparse_flops"] / (mean["sparse"] * 1e-3) / 1e12
-    tf_dense = alg["dense_flops"] / (mean["dense"] * 1e-3) / 1e12
-    pool_gbs = alg["pool_bytes"] / (mean["pool"] * 1e-3) / 1e9
+    head = summarize(cfg, per, kv_sum, peaks)
+    tf_sparse, tf_dense = head["sparse_tflops"], head["dense_tflops"]
     peak_tf = peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"])
     gather_gbs = alg["gather_bytes"] / (mean["sparse"] * 1e-3) / 1e9
-    lts_peak_gbs = 64.0 * 148 * (clk.get("sm_mhz") or peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e9
+    sm_mhz = (run.clocks.get("sparse_phase") or {}).get("sm_mhz") or clk.get("sm_mhz") or 1965.0
+    lts_peak_gbs = 64.0 * 148 * sm_mhz * 1e6 / 1e9
+    n_sparse_launches = 5 if args.policy.startswith("router") else 4
     line = {
         "metric": METRIC, "value": sparse_ms, "unit": "ms", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": False, "scaling": "weak",
@@ -396,15 +512,15 @@ def run_gpu(args):
         "data": "synthetic",
         "config": workload_config(cfg, args),
         "tokens_per_s": cfg.seqlen * world / (sparse_ms * 1e-3),
-        "x_dense": sparse_ms / mean["dense"],
-        "x_dense_kernel_only": mean["sparse"] / mean["dense"],
+        "x_dense": head["x_dense"],
+        "x_dense_kernel_only": head["x_dense_kernel_only"],
+        "x_dense_interleaved": head.get("x_dense_interleaved"),
         "stages_ms": {"pool": mean["pool"], "select": mean["select"], "sparse_attn": mean["sparse"],
                       "dense_attn": mean["dense"]},
-        "stages_ms_min": {"pool": best["pool"], "select": best["select"], "sparse_attn": best["sparse"],
-                          "dense_attn": best["dense"]},
+        "stats": head["stats"],
         "wall_ms_timed_region": wall_ms,
         "kv_count_sum": kv_sum,
-        "mean_blocks_per_tile": kv_sum / (cfg.n_q_heads * cfg.n_blocks),
+        "mean_blocks_per_tile": head["mean_blocks_per_tile"],
         "roofline": {"bound": "tensor", "kernel": "attn_kernel<sparse> (bsa_sparse_attn_fwd)",
                      "achieved": tf_sparse, "peak": peak_tf, "unit": "TFLOP/s", "frac": tf_sparse / peak_tf,
                      "traffic": ncu_traffic(f"attn_sparse/{args.workload}/{args.policy}"),
@@ -417,76 +533,85 @@ def run_gpu(args):
         "roofline_l2_gather": {"bound": "l2", "achieved": gather_gbs, "peak": lts_peak_gbs, "unit": "GB/s",
                                "frac": gather_gbs / lts_peak_gbs,
                                "bytes_per_launch": alg["gather_bytes"],
-                               "peak_source": "64 B/clk/SM x 148 SMs x measured SM clock "
+                               "peak_source": "64 B/clk/SM x 148 SMs x SM clock of the sparse phase "
                                               "(TMA-only ablation of the same kernel reached it)"},
         "roofline_dense": {"bound": "tensor", "achieved": tf_dense, "peak": peak_tf, "unit": "TFLOP/s",
                            "frac": tf_dense / peak_tf},
-        "roofline_pool": {"bound": "hbm", "achieved": pool_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                          "frac": pool_gbs / peaks["hbm_gbs"], "algorithmic_bytes": alg["pool_bytes"],
-                          "note": "cold L2 (flushed before the step)"},
+        "roofline_pool": {"bound": "hbm", "achieved": head["pool_gbs"], "peak": peaks["hbm_gbs"],
+                          "unit": "GB/s", "frac": head["pool_frac_of_hbm_peak"],
+                          "algorithmic_bytes": alg["pool_bytes"], "note": "cold L2 (flushed before the step)"},
         "e2e": {"value": e2e_ms, "unit": "ms", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
-        "gpu_launches": (args.steps) * (5 if args.policy.startswith("router") else 4)
-                        + args.steps,     # + the dense kernel of every step
+        # launches of libbsa kernels inside the timed region: K sparse passes (pool, score, route[,
+        # finalize], attention), K dense, and the interleaved-order passes
+        "gpu_launches": args.steps * (n_sparse_launches + 1) + min(3, args.steps) * (n_sparse_launches + 1),
         "clocks": clk,
     }
 
-    # ---- the long-context ratio regime (BASELINE.json configs[2]): 64K / 128K, few steps ------------
-    if not args.no_extra and args.workload == "C2" and world == 1:
-        extra = {}
+    # ---- the other BASELINE.json configs and the paper's own sweeps (fewer steps each) ------------------
+    if not args.no_extra and world == 1:
+        from dataclasses import replace
         del run
         torch.cuda.empty_cache()
-        for name, pols in (("C3a", ("router_quest", "topk")), ("C3b", ("router_quest", "topk")),
-                           ("C4", ("router_quest", "quest")), ("C5", ("router_quest", "router"))):
+        extra, sweeps = {}, {}
+        n_x, w_x = max(3, min(args.steps, 8)), 2
+        plans = [("C2", ("router_quest", "topk", "quest", "router")), ("C3a", ("router_quest", "topk")),
+                 ("C3b", ("topk",)), ("C4", ("router_quest", "quest")), ("C5", ("router_quest", "router")),
+                 ("C3c", ("router_quest", "topk"))]
+        for name, pols in plans:
             c = synth.CONFIGS[name]
-            i2 = synth.make_inputs(c)
+            i2 = inp if name == args.workload else synth.make_inputs(c)
+            dense_per = None
             for pol in pols:
+                if name == args.workload and pol == args.policy:
+                    continue
                 r2 = Runner(c, i2, pol, args.q_frac, torch, bsa)
-                m2, _ = r2.timed_steps(3, 1, with_dense=(pol == "router_quest"))   # dense once per config
-                if pol == "router_quest":
-                    dense_ms = m2["dense"]
-                s = m2["pool"] + m2["select"] + m2["sparse"]
-                kvs = int(r2.sel["kv_count"].sum().item())
-                a2 = algorithmic(c, kvs)
-                extra[f"{name}/{pol}"] = {
-                    "seqlen": c.seqlen, "sparse_path_ms": s, "pool_ms": m2["pool"], "select_ms": m2["select"],
-                    "sparse_attn_ms": m2["sparse"], "dense_attn_ms": dense_ms, "x_dense": s / dense_ms,
-                    "pool_gbs": a2["pool_bytes"] / (m2["pool"] * 1e-3) / 1e9,
-                    "sparse_tflops": a2["sparse_flops"] / (m2["sparse"] * 1e-3) / 1e12,
-                    "dense_tflops": a2["dense_flops"] / (dense_ms * 1e-3) / 1e12}
+                # the dense kernel once per config (at 256K it alone is ~0.5 s per pass: 2 passes)
+                want_dense = dense_per is None and not (name == args.workload)
+                p2 = r2.timed_steps(2 if name == "C3c" else n_x, w_x, with_dense=want_dense, clocks_index=local)
+                if want_dense:
+                    dense_per = p2["dense"]
+                elif dense_per is not None:
+                    p2["dense"] = dense_per
+                elif name == args.workload:
+                    p2["dense"] = per["dense"]
+                rec = summarize(c, p2, int(r2.sel["kv_count"].sum().item()), peaks)
+                rec["clocks"] = r2.clocks
+                extra[f"{name}/{pol}"] = rec
                 del r2
                 torch.cuda.empty_cache()
-        line["long_context"] = extra
-
-    # ---- the sweeps the paper itself varies (L123, L241-252), timing only ---------------
-    if args.sweep and world == 1:
-        from dataclasses import replace
-        try:
-            del run
-        except NameError:
-            pass
-        torch.cuda.empty_cache()
-        sweeps = {}
-        for kb, pol, qf in ([(kb, "router_quest", 0.25) for kb in (33, 40, 47, 52, 66)] +
-                            [(kb, "quest", 0.0) for kb in (33, 66)] +
-                            [(cfg.k_budget, "router_quest", qf) for qf in (0.1, 0.2, 0.3, 0.4)]):
-            c = replace(cfg, k_budget=kb)
-            r2 = Runner(c, inp, pol, qf, torch, bsa)
-            m2, _ = r2.timed_steps(3, 1, with_dense=False)
-            kvs = int(r2.sel["kv_count"].sum().item())
-            a2 = algorithmic(c, kvs)
-            sweeps[f"k={kb}/{pol}/q={qf}"] = {
-                "sparse_path_ms": m2["pool"] + m2["select"] + m2["sparse"], "select_ms": m2["select"],
-                "sparse_attn_ms": m2["sparse"], "mean_blocks_per_tile": kvs / (c.n_q_heads * c.n_blocks),
-                "sparse_tflops": a2["sparse_flops"] / (m2["sparse"] * 1e-3) / 1e12}
-            del r2
-            torch.cuda.empty_cache()
-        line["sweeps"] = sweeps
+            if name == "C2":   # k_budget in {33..66} (Table 4), q in {.1...4} (L123)
+                for kb, pol, qf in ([(kb, "router_quest", 0.4) for kb in (33, 40, 47, 52, 66)] +
+                                    [(kb, "quest", 0.0) for kb in (33, 66)] +
+                                    [(33, "router_quest", qf) for qf in (0.1, 0.2, 0.3)]):
+                    r2 = Runner(replace(c, k_budget=kb), i2, pol, qf, torch, bsa)
+                    p2 = r2.timed_steps(3, 1, with_dense=False)
+                    p2["dense"] = dense_per
+                    rec = summarize(replace(c, k_budget=kb), p2, int(r2.sel["kv_count"].sum().item()), peaks)
+                    rec.pop("stats")
+                    sweeps[f"k={kb}/{pol}/q={qf}"] = rec
+                    del r2
+                    torch.cuda.empty_cache()
+            del i2
+        line["extra"] = {"configs": extra, "sweeps": sweeps,
+                         "note": f"{n_x} timed steps after {w_x} warm-ups per entry (C3c: 2), dense kernel timed "
+                                 "once per config; sweeps at C2 (32K), 3 steps"}
 
     # ---- CPU oracle on this host's cores --------------------------------------------------------------
     import oracle
-    cpu_ms, cpu_s, text = oracle_sample_ms(cfg, inp, args.policy, args.q_frac, 16)
-    line["cpu_baseline"] = {"value": cpu_ms, "unit": "ms", "cores": oracle.max_threads(), "kind": "oracle",
-                            "sample": text, "cpu_seconds_spent": cpu_s}
+    cores = oracle.max_threads()
+    work = cfg.n_blocks * (cfg.n_blocks + 1) / 2 * cfg.block * cfg.head_dim * cfg.n_q_heads * 4.0
+    stride = int(min(512, max(1, 2 ** math.ceil(math.log2(max(work / (1.2e8 * cores * 25.0), 1))))))
+    cb = oracle_sample_ms(cfg, inp, args.policy, args.q_frac, stride)
+    line["cpu_baseline"] = {"value": cb["value"], "unit": "ms", "cores": cores, "kind": "oracle",
+                            "sample": cb["sample"], "measured_ms": cb["measured_ms"], "scale": cb["scale"],
+                            "extrapolated": cb["extrapolated"], "cpu_seconds_spent": cb["seconds"]}
+    if args.workload != "C2" and not args.no_extra and world == 1:
+        # the sparse pipeline timed IN FULL where that is affordable (C2, 32K)
+        c2 = synth.CONFIGS["C2"]
+        cb2 = oracle_sample_ms(c2, synth.make_inputs(c2), args.policy, args.q_frac, 1)
+        line["cpu_baseline_c2_full"] = {"value": cb2["value"], "unit": "ms", "cores": cores, "kind": "oracle",
+                                        "sample": cb2["sample"], "extrapolated": False,
+                                        "cpu_seconds_spent": cb2["seconds"]}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -497,13 +622,12 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="C2")
+    ap.add_argument("--workload", default="C3b")
     ap.add_argument("--policy", default="router_quest")
     ap.add_argument("--q-frac", type=float, default=0.25)
     ap.add_argument("--impl", default="bsa", choices=["bsa", "reference"])
-    ap.add_argument("--no-extra", action="store_true", help="skip the 64K / 128K ratio runs")
-    ap.add_argument("--sweep", action="store_true",
-                    help="also time the k_budget / q_frac sweeps of the paper (L123, L241-252)")
+    ap.add_argument("--no-extra", action="store_true",
+                    help="skip the other configs, the k_budget / q_frac sweeps and the full C2 oracle run")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

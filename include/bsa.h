@@ -16,7 +16,10 @@
  *     between calls.  `shape` is a HOST pointer.  `stream` is a cudaStream_t passed as void*.
  *   - Every call only enqueues work on `stream`; it never synchronises and never touches the
  *     default stream.
- *   - Argument checks run on the host before any launch; on a non-zero status nothing was enqueued.
+ *   - Argument checks run on the host before any launch: BSA_ERR_INVALID_ARG, BSA_ERR_UNSUPPORTED and
+ *     BSA_ERR_WORKSPACE_TOO_SMALL mean nothing was enqueued.  BSA_ERR_CUDA reports a failed CUDA call;
+ *     when it comes from a kernel launch of a multi-kernel call (bsa_select), the kernels launched
+ *     before it stay enqueued and the outputs are partially written.
  *     bsa_last_error() returns a thread-local description of the last failure.
  *   - Tensors are bf16 with the head dimension contiguous; strides are in elements.  Q and O share
  *     strides; K and V share strides.  Pointers and row strides must be 16-byte aligned.
@@ -51,6 +54,7 @@ typedef enum {
 } bsa_policy;
 
 enum { BSA_META_MEAN = 1, BSA_META_MINMAX = 2 }; /* bit mask for `kinds` */
+enum { BSA_META_SPLIT = 4 };                      /* bsa_block_meta_offset only: the bf16 split planes */
 #define BSA_RHO 2                                 /* expansion factor rho (L129) */
 
 typedef struct {
@@ -60,16 +64,23 @@ typedef struct {
 } bsa_shape;
 
 /*
- * Block metadata buffer ("meta"), documented so tests can read it:
+ * Block metadata buffer ("meta"), documented so tests can read and write it:
  *   offset 0                      : kmean fp32 [B, Hkv, N_B, d]   (Eq.1: (1/BLOCK_N) sum_j k_j)
  *   offset bsa_block_meta_offset(shape, BSA_META_MINMAX)
  *                                 : kmin  bf16 [B, Hkv, N_B, d]   (Eq.2: element-wise min)
  *   directly after kmin           : kmax  bf16 [B, Hkv, N_B, d]   (Eq.2: element-wise max)
- * The three planes have fixed offsets regardless of `kinds`; planes not requested are left untouched.
+ *   offset bsa_block_meta_offset(shape, BSA_META_SPLIT)
+ *                                 : three bf16 planes hi, mid, lo, each [B, Hkv, N_B, d], with
+ *                                   hi = bf16_rn(kmean), mid = bf16_rn(kmean - hi),
+ *                                   lo = bf16_rn(kmean - hi - mid), so hi + mid + lo == kmean exactly.
+ *                                   Written together with kmean (BSA_META_MEAN).  THE K-MEAN POLICIES OF
+ *                                   bsa_select READ THESE PLANES (tensor-core operands), not the fp32
+ *                                   kmean plane: a caller that overwrites kmean must rewrite the split.
+ * The planes have fixed offsets regardless of `kinds`; planes not requested are left untouched.
  * bsa_block_meta_bytes returns the size to allocate (0 on invalid shape).
  */
 size_t bsa_block_meta_bytes(const bsa_shape* shape, int kinds);
-size_t bsa_block_meta_offset(const bsa_shape* shape, int kind /* BSA_META_MEAN | BSA_META_MINMAX */);
+size_t bsa_block_meta_offset(const bsa_shape* shape, int kind /* BSA_META_MEAN | _MINMAX | _SPLIT */);
 
 /* Pools K once (one pass, 128-bit loads) into `meta`.  kinds: BSA_META_MEAN | BSA_META_MINMAX. */
 bsa_status bsa_build_block_meta(const bsa_shape* shape, const void* K, int kinds, void* meta,
@@ -99,6 +110,11 @@ size_t bsa_select_workspace_bytes(const bsa_shape* shape, bsa_policy policy, int
  * Outputs: kv_idx [B,Hq,Q_t,W] int32, kv_count [B,Hq,Q_t] int32, sigma [B,Hq,Q_t] fp32 (required);
  *          sigma_bar [B,Q_t] fp32, trigger [B,Q_t] u8, tau [B] fp32 (each may be NULL).
  * `meta` must hold the planes the policy needs (MEAN for TOPK/ROUTER, MINMAX for QUEST policies).
+ * Limits: 3 <= k_budget <= 128; N_B <= 8192 and N_B * 4 bytes of score row per head must fit the SM's
+ * shared memory beside the query planes (the error text states the largest N_B that fits; block 64 /
+ * head_dim 128 reaches N_B = 8192 = 512K tokens with both backbones).
+ * sigma_bar / trigger may be NULL only if `workspace` (bsa_select_workspace_bytes, 256-byte aligned
+ * use) is given: they are then kept there.
  */
 bsa_status bsa_select(const bsa_shape* shape, const void* Q, const void* meta, bsa_policy policy,
                       int32_t k_budget, double q_frac, int32_t* kv_idx, int32_t* kv_count,
@@ -106,10 +122,42 @@ bsa_status bsa_select(const bsa_shape* shape, const void* Q, const void* meta, b
                       size_t workspace_bytes, void* stream);
 
 /*
+ * D.4 diagnostics (App. D.4; Eq.18; (A1)/(A2) L431-432), computed
+ * from the tile scores while they are on chip.  bsa_select_diag = bsa_select with the same arguments and
+ * results, plus, per cell (tile t, head h) with at least rho*k + 1 visible blocks (L493; NaN elsewhere),
+ * with s~ the sorted list of Eq.10 (forced blocks on top, f of them):
+ *   g  [B,Hq,Q_t] = s~[k-1] - s~[k]        cutoff gap
+ *   G  [B,Hq,Q_t] = s~[k-1] - s~[rho k]    expansion gap
+ *   r  [B,Hq,Q_t] = s~[f]   - s~[k]        spread (so sigma = g / r, reading G1)
+ *   d2 [B,Hq,Q_t] = min over ranks j in [f, rho k), j != k-1, of s~[j] - s~[j+1]   (secondary spacing, A1)
+ * and for EVERY cell
+ *   rough [B,Hq,Q_t] = sum over visible blocks b and adjacent rows i, i+1 of tile t of
+ *                      (s[i+1,h,b] - s[i,h,b])^2      (step 3 of the recipe: E = 2 tau^2)
+ * and per sequence summary [B, BSA_DIAG_SUMMARY_LEN] fp32 (index: meaning), population = the valid cells:
+ *   0 n | 1 r_bar | 2 CV(r) = sqrt(Var r)/r_bar | 3 sigma_(q) = tau of the router (NaN otherwise) |
+ *   4 gamma_q = sigma_(q) r_bar | 5 band mass m_q(beta): fraction with g in gamma_q[1-beta,1+beta],
+ *   beta = CV(r) (Remark 1) | 6 / 7 10 % / 50 % order statistics of d2 (ceil(p n - 1e-9)-th smallest) |
+ *   8 tau_hat = sqrt(sum rough / (2 #pairs)) over all cells | 9 fraction with g == 0 |
+ *   10 g_q^+ = 40th percentile of g on {g > 0} (L501) | 11 g_q^+ / tau_hat | 12.. 0
+ * All pointers of bsa_diag_out are device pointers owned by the caller and must not be NULL; tau must
+ * not be NULL.
+ */
+#define BSA_DIAG_SUMMARY_LEN 16
+typedef struct {
+  float *g, *G, *r, *d2, *rough; /* each [B,Hq,Q_t] */
+  float* summary;                /* [B, BSA_DIAG_SUMMARY_LEN] */
+} bsa_diag_out;
+
+bsa_status bsa_select_diag(const bsa_shape* shape, const void* Q, const void* meta, bsa_policy policy,
+                           int32_t k_budget, double q_frac, int32_t* kv_idx, int32_t* kv_count,
+                           float* sigma, float* sigma_bar, uint8_t* trigger, float* tau,
+                           const bsa_diag_out* diag, void* workspace, size_t workspace_bytes, void* stream);
+
+/*
  * Sparse attention.  For tile t, head h, row i: softmax over keys j <= i of the blocks listed in
  * kv_idx[b,h,t,0..kv_count) (kv_count may be NULL: all W slots are read), scale <= 0 means
  * 1/sqrt(head_dim).  Entries >= N_B (sentinel) or > t are skipped; the block equal to t gets the
- * causal diagonal mask; the order of entries is free; entries of one row must be distinct.
+ * causal diagonal mask; the order of entries is free; a block listed more than once is attended once.
  * O [B,Hq,N,d] bf16 (Q strides); lse [B,Hq,N] fp32 natural-log-sum-exp of the scaled logits, or NULL.
  */
 bsa_status bsa_sparse_attn_fwd(const bsa_shape* shape, const void* Q, const void* K, const void* V,
@@ -119,6 +167,38 @@ bsa_status bsa_sparse_attn_fwd(const bsa_shape* shape, const void* Q, const void
 /* Dense causal attention with the same kernel design (every visible block). */
 bsa_status bsa_dense_attn_fwd(const bsa_shape* shape, const void* Q, const void* K, const void* V,
                               float softmax_scale, void* O, float* lse, void* stream);
+
+/*
+ * Ragged batches (SURVEY 8(f).1 "varlen"): n_seqs sequences packed along the token axis, Q / O
+ * [Hq, total, d], K / V [Hkv, total, d] with shape.batch = 1 and shape.seqlen = total =
+ * cu_seqlens[n_seqs]; cu_seqlens is a HOST array of n_seqs + 1 offsets, cu_seqlens[0] = 0, every length a
+ * multiple of shape.block (0 allowed).  Each sequence is an independent problem: its own causal frame,
+ * block numbers local to the sequence (0 .. T_i - 1, sentinel T_i) and its own quantile threshold
+ * (reading G9).  The calls loop over the sequences on `stream` (one set of launches per sequence).
+ * Index and statistics tensors are SEQUENCE-MAJOR, sequence i first token s_i = cu_seqlens[i],
+ * first tile t_i = s_i / block, T_i tiles:
+ *   kv_idx   : [Hq, T_i, W] at element Hq * W * t_i      kv_count, sigma : [Hq, T_i] at Hq * t_i
+ *   sigma_bar, trigger : [T_i] at t_i                    tau : [n_seqs]
+ *   lse      : [Hq, N_i] at Hq * s_i
+ *   meta     : sequence i at the sum over j < i of bsa_block_meta_bytes(shape with seqlen = N_j, 3)
+ *              rounded up to 256 (bsa_block_meta_bytes_varlen returns the total)
+ * Errors as for the batch calls; a failing sequence leaves the earlier sequences enqueued.
+ */
+size_t bsa_block_meta_bytes_varlen(const bsa_shape* shape, const int32_t* cu_seqlens, int32_t n_seqs,
+                                   int kinds);
+bsa_status bsa_build_block_meta_varlen(const bsa_shape* shape, const int32_t* cu_seqlens, int32_t n_seqs,
+                                       const void* K, int kinds, void* meta, void* stream);
+bsa_status bsa_select_varlen(const bsa_shape* shape, const int32_t* cu_seqlens, int32_t n_seqs, const void* Q,
+                             const void* meta, bsa_policy policy, int32_t k_budget, double q_frac,
+                             int32_t* kv_idx, int32_t* kv_count, float* sigma, float* sigma_bar,
+                             uint8_t* trigger, float* tau, void* stream);
+bsa_status bsa_sparse_attn_fwd_varlen(const bsa_shape* shape, const int32_t* cu_seqlens, int32_t n_seqs,
+                                      const void* Q, const void* K, const void* V, const int32_t* kv_idx,
+                                      const int32_t* kv_count, int32_t kv_width, float softmax_scale, void* O,
+                                      float* lse, void* stream);
+bsa_status bsa_dense_attn_fwd_varlen(const bsa_shape* shape, const int32_t* cu_seqlens, int32_t n_seqs,
+                                     const void* Q, const void* K, const void* V, float softmax_scale, void* O,
+                                     float* lse, void* stream);
 
 /* Thread-local, static storage; never NULL. */
 const char* bsa_last_error(void);

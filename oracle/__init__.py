@@ -52,6 +52,12 @@ def _load():
         lib.orc_attn_pairs.argtypes = [vp, vp, vp, i64, i64, i64, i64, i64, vp, vp, i64, ci, dbl,
                                        vp, i64, vp, vp]
         lib.orc_attn_pairs.restype = None
+        lib.orc_diag_cells.argtypes = [vp, vp, i64, i64, i64, vp, vp, vp, vp]
+        lib.orc_diag_cells.restype = None
+        lib.orc_roughness.argtypes = [vp, vp, vp, vp, i64, i64, i64, i64, i64, ci, vp, i64, vp]
+        lib.orc_roughness.restype = None
+        lib.orc_diag_summary.argtypes = [vp, vp, vp, vp, i64, i64, i64, i64, ci, ctypes.c_float, vp]
+        lib.orc_diag_summary.restype = None
         lib.orc_max_threads.restype = ci
         _lib = lib
     return _lib
@@ -188,3 +194,55 @@ def attn_full(Q, K, V, block: int, kv_idx=None, kv_count=None, scale=None):
     pairs = np.array([(t, h) for h in range(H) for t in range(T)], np.int64)
     O, lse = attn_pairs(Q, K, V, block, pairs, kv_idx, kv_count, scale)
     return O.reshape(H, N, d), lse.reshape(H, N)
+
+
+# ---- D.4 diagnostics (Eq.18) ------------------------------------------------------
+DIAG_SUMMARY = ("n", "r_bar", "cv_r", "sigma_q", "gamma_q", "band_mass", "d2_q10", "d2_q50", "tau_hat",
+                "zero_gap_frac", "g_q40_pos", "g_q40_pos_over_tau_hat")
+
+
+def diag_cells(score_sorted: np.ndarray, tiles, k: int):
+    """Per-cell g, G, r, d2 (each [n_tiles, H]) from select_tiles()['score_sorted'] [n, H, 2k+1]."""
+    ss = _c(score_sorted, np.float32)
+    n, H, w = ss.shape
+    assert w == RHO * k + 1
+    tiles = _c(np.asarray(tiles), np.int64)
+    out = [np.empty((n, H), np.float32) for _ in range(4)]
+    _load().orc_diag_cells(_p(ss), _p(tiles), n, H, k, *[_p(a) for a in out])
+    return dict(g=out[0], G=out[1], r=out[2], d2=out[3])
+
+
+def roughness(Q, meta, block: int, policy: str, tiles):
+    """rough [n_tiles, H]: sum over visible blocks and adjacent rows of (s[i+1,b] - s[i,b])^2."""
+    Q = _c(Q, np.uint16)
+    kmean, kmin, kmax = meta
+    H, N, d = Q.shape
+    tiles = _c(np.asarray(tiles), np.int64)
+    out = np.empty((len(tiles), H), np.float32)
+    _load().orc_roughness(_p(Q), _p(_c(kmean, np.float32)), _p(_c(kmin, np.uint16)), _p(_c(kmax, np.uint16)),
+                          H, kmean.shape[0], N, d, block, POLICIES[policy], _p(tiles), len(tiles), _p(out))
+    return out
+
+
+def diag_summary(g, r, d2, rough, k: int, block: int, router: bool, tau: float):
+    """Per-layer aggregates (dict keyed by DIAG_SUMMARY) from per-cell arrays laid out [T, H]."""
+    g, r, d2, rough = (_c(a, np.float32) for a in (g, r, d2, rough))
+    T, H = g.shape
+    out = np.empty(16, np.float32)
+    _load().orc_diag_summary(_p(g), _p(r), _p(d2), _p(rough), T, H, k, block, 1 if router else 0,
+                             float(tau), _p(out))
+    return {name: float(out[i]) for i, name in enumerate(DIAG_SUMMARY)}, out
+
+
+def diag(Q, meta, block: int, policy: str, k: int, q_frac: float):
+    """Full D.4 pass of one sequence: cells [T, H], rough [T, H], summary."""
+    H, N, d = Q.shape
+    T = N // block
+    tiles = np.arange(T)
+    sel = select_tiles(Q, meta, block, policy, k, tiles)
+    cells = diag_cells(sel["score_sorted"], tiles, k)
+    rough = roughness(Q, meta, block, policy, tiles)
+    _, tau, _ = route(sel["sigma"], policy, q_frac)
+    router = policy in ("router", "router_quest") and tau >= 0
+    summ, vec = diag_summary(cells["g"], cells["r"], cells["d2"], rough, k, block, router, tau)
+    return dict(cells, rough=rough, summary=summ, summary_vec=vec, tau=tau)

@@ -16,6 +16,8 @@
  * margin examples E1..E5 (tests/golden/margin_examples.txt), sigma in [0,1] and affine invariance,
  * Quest upper bound (L54, L82), routed count = ceil(qT) (L426), Eq.15 closed form (L346),
  * k_budget >= N_B  =>  sparse == dense, dense == torch CPU SDPA (library routine).
+ * D.4 diagnostics (orc_diag_cells / orc_roughness / orc_diag_summary): hand-worked examples D1-D3
+ * (tests/golden/diag_examples.txt), closed forms (identical / alternating rows), numpy brute force.
  * Parity unpinned (conventions fixed by fiat): G5 (sigma := 1 when nothing is dropped),
  * G6 (tie-break: lower block index first), G7 (GQA mapping h -> h / (H/H_kv)), G9 (per-sequence
  * quantile; batch is looped by the caller).
@@ -316,6 +318,124 @@ void orc_attn_pairs(const uint16_t* Q, const uint16_t* K, const uint16_t* V, int
     }
     free(sel); free(logit); free(acc);
   }
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * D.4 diagnostics (App. D.4; definitions Eq.18; (A1)/(A2) L431-432;
+ * Remark 1 L480; Proposition 1; measured-quantities paragraph L493-501).  SURVEY 8(f).3.
+ *
+ * Per cell (tile t, head h), from the sorted list s~ of Eq.10 (score_sorted[0..2k], forced blocks on
+ * top as +inf, f of them; reading G1 puts the best NON-forced score in the place of s_(0)):
+ *     g = s~[k-1] - s~[k]      G = s~[k-1] - s~[rho k]      r = s~[f] - s~[k]      (fp32 subtractions)
+ *     d2 = min_{j = f .. rho k - 1, j != k-1} (s~[j] - s~[j+1])     secondary spacing (A1), on the
+ *          ranks the selection keeps on chip
+ * defined for cells with at least rho*k + 1 visible blocks (L493); NaN elsewhere.
+ *   score_sorted [n_tiles, H, 2k+1];  g, G, r, d2 [n_tiles, H]
+ * ------------------------------------------------------------------------------------------- */
+void orc_diag_cells(const float* score_sorted, const int64_t* tiles, int64_t n_tiles, int64_t H,
+                    int64_t k, float* g, float* G, float* r, float* d2) {
+  int64_t W2 = RHO * k;
+  for (int64_t it = 0; it < n_tiles; ++it)
+    for (int64_t h = 0; h < H; ++h) {
+      int64_t t = tiles[it], o = it * H + h;
+      const float* ss = score_sorted + o * (W2 + 1);
+      if (t + 1 < W2 + 1) { g[o] = G[o] = r[o] = d2[o] = NAN; continue; }
+      int64_t f = (t == 0) ? 1 : 2;
+      g[o] = ss[k - 1] - ss[k];
+      G[o] = ss[k - 1] - ss[W2];
+      r[o] = ss[f] - ss[k];
+      float mn = INFINITY;
+      for (int64_t j = f; j < W2; ++j) {
+        if (j == k - 1) continue;
+        float sp = ss[j] - ss[j + 1];
+        if (sp < mn) mn = sp;
+      }
+      d2[o] = mn;
+    }
+}
+
+/* Step 3 of the recipe (L489): row-to-row roughness of the per-row block scores,
+ *     rough[t,h] = sum_{b <= t} sum_{i = 0}^{Bn-2} (s[tBn+i+1, h, b] - s[tBn+i, h, b])^2
+ * with s the fp32 row scores of O3 / O3q; pairs of adjacent rows inside one tile only (reading G19).
+ * Accumulated in double, rounded once.   rough [n_tiles, H] */
+void orc_roughness(const uint16_t* Q, const float* kmean, const uint16_t* kmin, const uint16_t* kmax,
+                   int64_t H, int64_t Hkv, int64_t N, int64_t d, int64_t Bn, int policy,
+                   const int64_t* tiles, int64_t n_tiles, float* rough) {
+  int64_t NB = N / Bn, G = H / Hkv;
+  int quest = (policy == POLICY_QUEST || policy == POLICY_ROUTER_QUEST);
+#pragma omp parallel for collapse(2) schedule(dynamic, 1)
+  for (int64_t it = 0; it < n_tiles; ++it)
+    for (int64_t h = 0; h < H; ++h) {
+      int64_t t = tiles[it], g = h / G;
+      double acc = 0.0;
+      for (int64_t b = 0; b <= t; ++b) {
+        int64_t o = (g * NB + b) * d;
+        float prev = 0.0f;
+        for (int64_t i = 0; i < Bn; ++i) {
+          const uint16_t* q = Q + (h * N + t * Bn + i) * d;
+          float s = quest ? row_score_quest(q, kmin + o, kmax + o, d) : row_score_mean(q, kmean + o, d);
+          if (i > 0) { double df = (double)s - (double)prev; acc += df * df; }
+          prev = s;
+        }
+      }
+      rough[it * H + h] = (float)acc;
+    }
+}
+
+/* Per-layer aggregates over the valid cells (t >= rho k), see include/bsa.h for the index list:
+ *  0 n | 1 r_bar | 2 CV(r) (population variance, A2) | 3 sigma_(q) = tau | 4 gamma_q = sigma_(q) r_bar |
+ *  5 band mass m_q(beta), beta = CV(r) (Remark 1) | 6, 7 10 % / 50 % order statistics of d2 |
+ *  8 tau_hat = sqrt(sum rough / (2 #pairs)) over ALL cells, #pairs = H T(T+1)/2 (Bn-1) |
+ *  9 fraction g == 0 | 10 g_q^+ = 40th percentile of g on {g > 0} (L501) | 11 g_q^+ / tau_hat
+ * Order statistic: the ceil(p n - 1e-9)-th smallest (as reading G3).
+ * Inputs laid out [T, H] (all tiles of one sequence). */
+void orc_diag_summary(const float* g, const float* r, const float* d2, const float* rough, int64_t T,
+                      int64_t H, int64_t k, int64_t Bn, int router, float tau, float* out /* [16] */) {
+  int64_t t_min = RHO * k;
+  int64_t n = (T > t_min) ? H * (T - t_min) : 0;
+  for (int i = 0; i < 16; ++i) out[i] = (i < 12) ? NAN : 0.0f;
+  double rs = 0.0;
+  for (int64_t i = 0; i < T * H; ++i) rs += (double)rough[i];
+  double pairs = (double)H * ((double)T * (double)(T + 1) / 2.0) * (double)(Bn - 1);
+  double tau_hat = sqrt(rs / (2.0 * pairs));
+  out[0] = (float)n;
+  out[8] = (float)tau_hat;
+  if (n == 0) return;
+  double sum = 0.0;
+  for (int64_t t = t_min; t < T; ++t) for (int64_t h = 0; h < H; ++h) sum += (double)r[t * H + h];
+  double r_bar = sum / (double)n, var = 0.0;
+  for (int64_t t = t_min; t < T; ++t) for (int64_t h = 0; h < H; ++h) {
+    double dv = (double)r[t * H + h] - r_bar; var += dv * dv;
+  }
+  var /= (double)n;
+  double cv = sqrt(var) / r_bar;
+  out[1] = (float)r_bar; out[2] = (float)cv;
+  float* gv = (float*)malloc(sizeof(float) * (size_t)n);
+  float* dv2 = (float*)malloc(sizeof(float) * (size_t)n);
+  int64_t c = 0, npos = 0, nzero = 0, band = 0;
+  double gamma = (double)tau * r_bar, lo = gamma * (1.0 - cv), hi = gamma * (1.0 + cv);
+  for (int64_t t = t_min; t < T; ++t) for (int64_t h = 0; h < H; ++h) {
+    float x = g[t * H + h];
+    dv2[c++] = d2[t * H + h];
+    if (x == 0.0f) ++nzero;
+    if (x > 0.0f) gv[npos++] = x;
+    if (router && (double)x >= lo && (double)x <= hi) ++band;
+  }
+  if (router) { out[3] = tau; out[4] = (float)gamma; out[5] = (float)((double)band / (double)n); }
+  qsort(dv2, (size_t)n, sizeof(float), float_cmp);
+  int64_t m10 = (int64_t)ceil(0.10 * (double)n - 1e-9), m50 = (int64_t)ceil(0.50 * (double)n - 1e-9);
+  if (m10 < 1) m10 = 1;
+  if (m50 < 1) m50 = 1;
+  out[6] = dv2[m10 - 1]; out[7] = dv2[m50 - 1];
+  out[9] = (float)((double)nzero / (double)n);
+  if (npos > 0) {
+    qsort(gv, (size_t)npos, sizeof(float), float_cmp);
+    int64_t m40 = (int64_t)ceil(0.40 * (double)npos - 1e-9);
+    if (m40 < 1) m40 = 1;
+    out[10] = gv[m40 - 1];
+    out[11] = (float)((double)gv[m40 - 1] / tau_hat);
+  }
+  free(gv); free(dv2);
 }
 
 int orc_max_threads(void) {

@@ -14,7 +14,10 @@ import torch
 from .build import LIB, build_lib
 
 BSA_OK = 0
-BSA_META_MEAN, BSA_META_MINMAX = 1, 2
+BSA_META_MEAN, BSA_META_MINMAX, BSA_META_SPLIT = 1, 2, 4
+BSA_DIAG_SUMMARY_LEN = 16
+DIAG_SUMMARY = ("n", "r_bar", "cv_r", "sigma_q", "gamma_q", "band_mass", "d2_q10", "d2_q50", "tau_hat",
+                "zero_gap_frac", "g_q40_pos", "g_q40_pos_over_tau_hat")
 BSA_RHO = 2
 POLICIES = {"topk": 0, "router": 1, "quest": 2, "router_quest": 3}
 STATUS = {0: "BSA_OK", 1: "BSA_ERR_INVALID_ARG", 2: "BSA_ERR_UNSUPPORTED",
@@ -27,6 +30,10 @@ class BsaShape(ctypes.Structure):
                 ("q_stride_b", ctypes.c_int64), ("q_stride_h", ctypes.c_int64),
                 ("q_stride_n", ctypes.c_int64), ("kv_stride_b", ctypes.c_int64),
                 ("kv_stride_h", ctypes.c_int64), ("kv_stride_n", ctypes.c_int64)]
+
+
+class BsaDiagOut(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_void_p) for n in ("g", "G", "r", "d2", "rough", "summary")]
 
 
 class BsaError(RuntimeError):
@@ -44,8 +51,8 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     if _lib is not None and path is None:
         return _lib
     p = path or LIB
-    if not os.path.exists(p):
-        build_lib()  # raises if nvcc is missing or the build fails
+    if path is None:
+        build_lib()  # no-op when libbsa.so matches the sources (hash); raises if the build fails
     lib = ctypes.CDLL(p)
     vp, sz, i32, sp = ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int32, ctypes.POINTER(BsaShape)
     lib.bsa_block_meta_bytes.argtypes = [sp, ctypes.c_int]
@@ -61,10 +68,25 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     lib.bsa_select.argtypes = [sp, vp, vp, ctypes.c_int, i32, ctypes.c_double, vp, vp, vp, vp, vp, vp,
                                vp, sz, vp]
     lib.bsa_select.restype = ctypes.c_int
+    lib.bsa_select_diag.argtypes = [sp, vp, vp, ctypes.c_int, i32, ctypes.c_double, vp, vp, vp, vp, vp, vp,
+                                    ctypes.POINTER(BsaDiagOut), vp, sz, vp]
+    lib.bsa_select_diag.restype = ctypes.c_int
     lib.bsa_sparse_attn_fwd.argtypes = [sp, vp, vp, vp, vp, vp, i32, ctypes.c_float, vp, vp, vp]
     lib.bsa_sparse_attn_fwd.restype = ctypes.c_int
     lib.bsa_dense_attn_fwd.argtypes = [sp, vp, vp, vp, ctypes.c_float, vp, vp, vp]
     lib.bsa_dense_attn_fwd.restype = ctypes.c_int
+    ip = ctypes.POINTER(ctypes.c_int32)
+    lib.bsa_block_meta_bytes_varlen.argtypes = [sp, ip, i32, ctypes.c_int]
+    lib.bsa_block_meta_bytes_varlen.restype = sz
+    lib.bsa_build_block_meta_varlen.argtypes = [sp, ip, i32, vp, ctypes.c_int, vp, vp]
+    lib.bsa_build_block_meta_varlen.restype = ctypes.c_int
+    lib.bsa_select_varlen.argtypes = [sp, ip, i32, vp, vp, ctypes.c_int, i32, ctypes.c_double, vp, vp, vp, vp,
+                                      vp, vp, vp]
+    lib.bsa_select_varlen.restype = ctypes.c_int
+    lib.bsa_sparse_attn_fwd_varlen.argtypes = [sp, ip, i32, vp, vp, vp, vp, vp, i32, ctypes.c_float, vp, vp, vp]
+    lib.bsa_sparse_attn_fwd_varlen.restype = ctypes.c_int
+    lib.bsa_dense_attn_fwd_varlen.argtypes = [sp, ip, i32, vp, vp, vp, ctypes.c_float, vp, vp, vp]
+    lib.bsa_dense_attn_fwd_varlen.restype = ctypes.c_int
     lib.bsa_last_error.restype = ctypes.c_char_p
     lib.bsa_version.restype = ctypes.c_char_p
     if path is None:
@@ -133,15 +155,29 @@ def meta_views(meta: torch.Tensor, K_shape, block: int):
     return kmean, kmin, kmax
 
 
+def meta_split_view(meta: torch.Tensor, K_shape, block: int):
+    """The three bf16 planes hi, mid, lo (hi + mid + lo == kmean) as one view [3, B, Hkv, N_B, d]."""
+    B, Hkv, N, d = K_shape
+    NB = N // block
+    n = B * Hkv * NB * d
+    s = BsaShape(B, N, Hkv, Hkv, d, block, Hkv * N * d, N * d, d, Hkv * N * d, N * d, d)
+    off = int(load_library().bsa_block_meta_offset(ctypes.byref(s), BSA_META_SPLIT))
+    return meta[off:off + 6 * n].view(torch.bfloat16).view(3, B, Hkv, NB, d)
+
+
 def bsa_kv_width(policy: str, k_budget: int) -> int:
     return int(load_library().bsa_kv_width(POLICIES[policy], k_budget))
 
 
 def bsa_select(Q: torch.Tensor, meta: torch.Tensor, K_like: torch.Tensor, block: int, policy: str,
-               k_budget: int, q_frac: float, out: dict | None = None) -> dict:
+               k_budget: int, q_frac: float, out: dict | None = None, diag: bool = False,
+               use_workspace: bool = False) -> dict:
     """Selection.  K_like only provides the K/V shape and strides.  Returns a dict with kv_idx
     [B,Hq,T,W] int32, kv_count [B,Hq,T] int32, sigma [B,Hq,T] f32, sigma_bar [B,T] f32,
-    trigger [B,T] u8, tau [B] f32.  `out` may carry preallocated tensors of those names."""
+    trigger [B,T] u8, tau [B] f32.  `out` may carry preallocated tensors of those names.
+    diag=True calls bsa_select_diag and adds g, G, r, d2, rough [B,Hq,T] f32 and summary [B,16] f32.
+    use_workspace=True passes sigma_bar = trigger = NULL and a workspace buffer instead (the results
+    then stay inside the library's workspace; `sigma_bar` / `trigger` are absent from the dict)."""
     lib = load_library()
     shape = make_shape(Q, K_like, block)
     B, H, N, _ = Q.shape
@@ -152,12 +188,27 @@ def bsa_select(Q: torch.Tensor, meta: torch.Tensor, K_like: torch.Tensor, block:
     o.setdefault("kv_idx", torch.empty((B, H, T, max(W, 1)), dtype=torch.int32, device=dev))
     o.setdefault("kv_count", torch.empty((B, H, T), dtype=torch.int32, device=dev))
     o.setdefault("sigma", torch.empty((B, H, T), dtype=torch.float32, device=dev))
-    o.setdefault("sigma_bar", torch.empty((B, T), dtype=torch.float32, device=dev))
-    o.setdefault("trigger", torch.empty((B, T), dtype=torch.uint8, device=dev))
     o.setdefault("tau", torch.empty((B,), dtype=torch.float32, device=dev))
-    _check(lib.bsa_select(ctypes.byref(shape), _ptr(Q), _ptr(meta), POLICIES[policy], k_budget,
-                          float(q_frac), _ptr(o["kv_idx"]), _ptr(o["kv_count"]), _ptr(o["sigma"]),
-                          _ptr(o["sigma_bar"]), _ptr(o["trigger"]), _ptr(o["tau"]), None, 0, _stream()))
+    ws, ws_bytes = None, 0
+    if use_workspace:
+        ws_bytes = int(lib.bsa_select_workspace_bytes(ctypes.byref(shape), POLICIES[policy], k_budget))
+        ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
+        o["workspace"] = ws
+        sb, tr = None, None
+    else:
+        o.setdefault("sigma_bar", torch.empty((B, T), dtype=torch.float32, device=dev))
+        o.setdefault("trigger", torch.empty((B, T), dtype=torch.uint8, device=dev))
+        sb, tr = o["sigma_bar"], o["trigger"]
+    args = [ctypes.byref(shape), _ptr(Q), _ptr(meta), POLICIES[policy], k_budget, float(q_frac),
+            _ptr(o["kv_idx"]), _ptr(o["kv_count"]), _ptr(o["sigma"]), _ptr(sb), _ptr(tr), _ptr(o["tau"])]
+    if diag:
+        for n in ("g", "G", "r", "d2", "rough"):
+            o.setdefault(n, torch.empty((B, H, T), dtype=torch.float32, device=dev))
+        o.setdefault("summary", torch.empty((B, BSA_DIAG_SUMMARY_LEN), dtype=torch.float32, device=dev))
+        d = BsaDiagOut(*[_ptr(o[n]) for n in ("g", "G", "r", "d2", "rough", "summary")])
+        _check(lib.bsa_select_diag(*args, ctypes.byref(d), _ptr(ws), ws_bytes, _stream()))
+    else:
+        _check(lib.bsa_select(*args, _ptr(ws), ws_bytes, _stream()))
     o["W"] = W
     return o
 
@@ -192,6 +243,68 @@ def bsa_dense_attn_fwd(Q, K, V, block: int, softmax_scale: float = 0.0, O: torch
         lse = torch.empty(Q.shape[:3], dtype=torch.float32, device=Q.device)
     _check(lib.bsa_dense_attn_fwd(ctypes.byref(shape), _ptr(Q), _ptr(K), _ptr(V), float(softmax_scale),
                                   _ptr(O), _ptr(lse), _stream()))
+    return O, lse
+
+
+# ---- ragged batches: packed Q / O [1, Hq, total, d], K / V [1, Hkv, total, d] + cu_seqlens --------------
+def _cu(cu_seqlens):
+    arr = (ctypes.c_int32 * len(cu_seqlens))(*[int(x) for x in cu_seqlens])
+    return arr, len(cu_seqlens) - 1
+
+
+def bsa_build_block_meta_varlen(K: torch.Tensor, cu_seqlens, block: int, kinds: int = 3):
+    lib = load_library()
+    shape = make_shape(None, K, block)
+    cu, n = _cu(cu_seqlens)
+    nbytes = int(lib.bsa_block_meta_bytes_varlen(ctypes.byref(shape), cu, n, kinds))
+    meta = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=K.device)
+    _check(lib.bsa_build_block_meta_varlen(ctypes.byref(shape), cu, n, _ptr(K), kinds, _ptr(meta), _stream()))
+    return meta
+
+
+def bsa_select_varlen(Q, meta, K_like, cu_seqlens, block: int, policy: str, k_budget: int, q_frac: float):
+    """Sequence-major outputs (include/bsa.h "Ragged batches"): kv_idx flat [Hq * total_T * W],
+    kv_count / sigma flat [Hq * total_T], sigma_bar / trigger [total_T], tau [n_seqs]."""
+    lib = load_library()
+    shape = make_shape(Q, K_like, block)
+    cu, n = _cu(cu_seqlens)
+    H, total_T = Q.shape[1], Q.shape[2] // block
+    W = bsa_kv_width(policy, k_budget)
+    dev = Q.device
+    o = dict(kv_idx=torch.empty(H * total_T * W, dtype=torch.int32, device=dev),
+             kv_count=torch.empty(H * total_T, dtype=torch.int32, device=dev),
+             sigma=torch.empty(H * total_T, dtype=torch.float32, device=dev),
+             sigma_bar=torch.empty(total_T, dtype=torch.float32, device=dev),
+             trigger=torch.empty(total_T, dtype=torch.uint8, device=dev),
+             tau=torch.empty(n, dtype=torch.float32, device=dev), W=W)
+    _check(lib.bsa_select_varlen(ctypes.byref(shape), cu, n, _ptr(Q), _ptr(meta), POLICIES[policy], k_budget,
+                                 float(q_frac), _ptr(o["kv_idx"]), _ptr(o["kv_count"]), _ptr(o["sigma"]),
+                                 _ptr(o["sigma_bar"]), _ptr(o["trigger"]), _ptr(o["tau"]), _stream()))
+    return o
+
+
+def bsa_sparse_attn_fwd_varlen(Q, K, V, cu_seqlens, kv_idx, kv_count, kv_width: int, block: int,
+                               softmax_scale: float = 0.0, want_lse: bool = False):
+    lib = load_library()
+    shape = make_shape(Q, K, block)
+    cu, n = _cu(cu_seqlens)
+    O = torch.empty_like(Q)
+    lse = torch.empty(Q.shape[1] * Q.shape[2], dtype=torch.float32, device=Q.device) if want_lse else None
+    _check(lib.bsa_sparse_attn_fwd_varlen(ctypes.byref(shape), cu, n, _ptr(Q), _ptr(K), _ptr(V), _ptr(kv_idx),
+                                          _ptr(kv_count), kv_width, float(softmax_scale), _ptr(O), _ptr(lse),
+                                          _stream()))
+    return O, lse
+
+
+def bsa_dense_attn_fwd_varlen(Q, K, V, cu_seqlens, block: int, softmax_scale: float = 0.0,
+                              want_lse: bool = False):
+    lib = load_library()
+    shape = make_shape(Q, K, block)
+    cu, n = _cu(cu_seqlens)
+    O = torch.empty_like(Q)
+    lse = torch.empty(Q.shape[1] * Q.shape[2], dtype=torch.float32, device=Q.device) if want_lse else None
+    _check(lib.bsa_dense_attn_fwd_varlen(ctypes.byref(shape), cu, n, _ptr(Q), _ptr(K), _ptr(V),
+                                         float(softmax_scale), _ptr(O), _ptr(lse), _stream()))
     return O, lse
 
 

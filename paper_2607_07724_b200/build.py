@@ -7,6 +7,7 @@ repository snapshot.
 """
 from __future__ import annotations
 
+import hashlib
 import os
 import shlex
 import shutil
@@ -16,10 +17,14 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libbsa.so")
-SOURCES = ["api.cu", "pool.cu", "select.cu", "score_tc.cu", "attn.cu"]
+STAMP = LIB + ".srchash"
+SOURCES = ["api.cu", "pool.cu", "select.cu", "score_tc_quest.cu", "score_tc_mean.cu", "attn.cu", "diag.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 NVCC_FLAGS += shlex.split(os.environ.get("BSA_NVCC_FLAGS", ""))   # developer knob, e.g. -DBSA_TC_OCC2=0
+if os.environ.get("BSA_DEBUG_TRAP", "0") not in ("", "0"):
+    # debug builds only: a protocol bug traps after ~4 s of spinning on an mbarrier instead of hanging
+    NVCC_FLAGS.append("-DBSA_MBAR_TRAP=1")
 
 
 def _nvcc() -> str:
@@ -29,13 +34,26 @@ def _nvcc() -> str:
     raise RuntimeError("nvcc not found; libbsa cannot be built")
 
 
+def _src_hash() -> str:
+    """Hash of everything libbsa.so is built from: csrc/*, include/bsa.h and the nvcc flags.  mtimes
+    are not used -- a repository snapshot copied to another box need not keep them."""
+    h = hashlib.sha256()
+    files = sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC))
+    files.append(os.path.join(_HERE, "..", "include", "bsa.h"))
+    for f in files:
+        h.update(os.path.basename(f).encode())
+        with open(f, "rb") as fh:
+            h.update(fh.read())
+    h.update(" ".join(NVCC_FLAGS).encode())
+    return h.hexdigest()
+
+
 def _stale() -> bool:
-    if not os.path.exists(LIB):
+    """True when libbsa.so is missing or was not built from the sources as they are now."""
+    if not os.path.exists(LIB) or not os.path.exists(STAMP):
         return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
-    deps.append(os.path.join(_HERE, "..", "include", "bsa.h"))
-    return any(os.path.getmtime(d) > t for d in deps)
+    with open(STAMP) as f:
+        return f.read().strip() != _src_hash()
 
 
 def build_lib(force: bool = False, verbose: bool = False) -> str:
@@ -63,6 +81,8 @@ def build_lib(force: bool = False, verbose: bool = False) -> str:
         raise RuntimeError("nvcc failed while building libbsa.so")
     subprocess.check_call([nvcc, "-shared", "-o", LIB, *objs, "-gencode",
                            "arch=compute_100a,code=sm_100a"])
+    with open(STAMP, "w") as f:
+        f.write(_src_hash() + "\n")
     return LIB
 
 

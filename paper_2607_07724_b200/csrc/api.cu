@@ -118,7 +118,7 @@ size_t bsa_block_meta_offset(const bsa_shape* shape, int kind) {
   Dims D;
   if (make_dims(shape, &D) != BSA_OK) return 0;
   const MetaLayout L = meta_layout(D);
-  return kind == BSA_META_MINMAX ? L.off_min : L.off_mean;
+  return kind == BSA_META_MINMAX ? L.off_min : kind == BSA_META_SPLIT ? L.off_split : L.off_mean;
 }
 
 bsa_status bsa_build_block_meta(const bsa_shape* shape, const void* K, int kinds, void* meta,
@@ -148,10 +148,11 @@ size_t bsa_select_workspace_bytes(const bsa_shape* shape, bsa_policy policy, int
   return align_up(bt * 4, 256) + align_up(bt, 256) + 256;
 }
 
-bsa_status bsa_select(const bsa_shape* shape, const void* Q, const void* meta, bsa_policy policy,
-                      int32_t k_budget, double q_frac, int32_t* kv_idx, int32_t* kv_count,
-                      float* sigma, float* sigma_bar, uint8_t* trigger, float* tau, void* workspace,
-                      size_t workspace_bytes, void* stream) {
+static bsa_status select_common(const bsa_shape* shape, const void* Q, const void* meta, bsa_policy policy,
+                                int32_t k_budget, double q_frac, int32_t* kv_idx, int32_t* kv_count,
+                                float* sigma, float* sigma_bar, uint8_t* trigger, float* tau,
+                                const bsa_diag_out* diag, bool want_diag, void* workspace,
+                                size_t workspace_bytes, void* stream) {
   Dims D;
   bsa_status st = make_dims(shape, &D);
   if (st != BSA_OK) return st;
@@ -164,7 +165,14 @@ bsa_status bsa_select(const bsa_shape* shape, const void* Q, const void* meta, b
     return fail(BSA_ERR_INVALID_ARG, "q_frac %g outside [0, 1]", q_frac);
   if (!aligned16(Q) || (reinterpret_cast<uintptr_t>(meta) & 255u))
     return fail(BSA_ERR_INVALID_ARG, "Q must be 16-byte and meta 256-byte aligned");
-  if (D.NB > 8192) return fail(BSA_ERR_UNSUPPORTED, "more than 8192 blocks per sequence in select");
+  if (D.NB > 8192)
+    return fail(BSA_ERR_UNSUPPORTED, "select: %d blocks per sequence, at most 8192 are supported", D.NB);
+  SelectDiag dg = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  if (want_diag) {
+    if (!diag || !diag->g || !diag->G || !diag->r || !diag->d2 || !diag->rough || !diag->summary || !tau)
+      return fail(BSA_ERR_INVALID_ARG, "diagnostics: every bsa_diag_out pointer and tau must be given");
+    dg = {diag->g, diag->G, diag->r, diag->d2, diag->rough, diag->summary};
+  }
   const size_t need = bsa_select_workspace_bytes(shape, policy, k_budget);
   if ((!sigma_bar || !trigger) && (!workspace || workspace_bytes < need))
     return fail(BSA_ERR_WORKSPACE_TOO_SMALL, "workspace of %zu bytes needed, %zu given", need,
@@ -184,7 +192,24 @@ bsa_status bsa_select(const bsa_shape* shape, const void* Q, const void* meta, b
   }
   const int W = bsa_kv_width(policy, k_budget);
   return launch_select(D, Q, meta, policy, k_budget, W, m, kv_idx, kv_count, sigma, sigma_bar, trigger,
-                       tau, static_cast<cudaStream_t>(stream));
+                       tau, dg, static_cast<cudaStream_t>(stream));
+}
+
+bsa_status bsa_select(const bsa_shape* shape, const void* Q, const void* meta, bsa_policy policy,
+                      int32_t k_budget, double q_frac, int32_t* kv_idx, int32_t* kv_count,
+                      float* sigma, float* sigma_bar, uint8_t* trigger, float* tau, void* workspace,
+                      size_t workspace_bytes, void* stream) {
+  return select_common(shape, Q, meta, policy, k_budget, q_frac, kv_idx, kv_count, sigma, sigma_bar,
+                       trigger, tau, nullptr, false, workspace, workspace_bytes, stream);
+}
+
+bsa_status bsa_select_diag(const bsa_shape* shape, const void* Q, const void* meta, bsa_policy policy,
+                           int32_t k_budget, double q_frac, int32_t* kv_idx, int32_t* kv_count,
+                           float* sigma, float* sigma_bar, uint8_t* trigger, float* tau,
+                           const bsa_diag_out* diag, void* workspace, size_t workspace_bytes,
+                           void* stream) {
+  return select_common(shape, Q, meta, policy, k_budget, q_frac, kv_idx, kv_count, sigma, sigma_bar,
+                       trigger, tau, diag, true, workspace, workspace_bytes, stream);
 }
 
 static bsa_status attn_common(const bsa_shape* shape, const void* Q, const void* K, const void* V,
@@ -215,6 +240,135 @@ bsa_status bsa_sparse_attn_fwd(const bsa_shape* shape, const void* Q, const void
 bsa_status bsa_dense_attn_fwd(const bsa_shape* shape, const void* Q, const void* K, const void* V,
                               float softmax_scale, void* O, float* lse, void* stream) {
   return attn_common(shape, Q, K, V, nullptr, nullptr, 0, false, softmax_scale, O, lse, stream);
+}
+
+/* ---- ragged batches (SURVEY 8(f).1 "varlen") ------------------------------------------------------
+ * A loop over the sequences on the caller's stream; every sequence is an independent batch-1 problem
+ * (own causal frame, own block numbering, own quantile -- reading G9). */
+static bsa_status varlen_check(const bsa_shape* shape, const int32_t* cu, int32_t n_seqs) {
+  if (!shape || !cu) return fail(BSA_ERR_INVALID_ARG, "shape or cu_seqlens is NULL");
+  if (n_seqs < 1) return fail(BSA_ERR_INVALID_ARG, "n_seqs %d < 1", n_seqs);
+  if (shape->batch != 1) return fail(BSA_ERR_INVALID_ARG, "varlen: shape.batch must be 1 (packed layout)");
+  if (shape->block != 64 && shape->block != 128)
+    return fail(BSA_ERR_UNSUPPORTED, "block %d not in {64, 128}", shape->block);
+  if (cu[0] != 0 || cu[n_seqs] != shape->seqlen)
+    return fail(BSA_ERR_INVALID_ARG, "cu_seqlens must run from 0 to shape.seqlen (%d)", shape->seqlen);
+  for (int i = 0; i < n_seqs; ++i) {
+    const int len = cu[i + 1] - cu[i];
+    if (len < 0 || len % shape->block != 0)
+      return fail(BSA_ERR_INVALID_ARG, "sequence %d: length %d is negative or not a multiple of block %d", i,
+                  len, shape->block);
+  }
+  return BSA_OK;
+}
+
+static bsa_shape sub_shape(const bsa_shape* shape, int len) {
+  bsa_shape s = *shape;
+  s.seqlen = len;
+  return s;
+}
+
+static size_t meta_bytes_padded(const bsa_shape* s, int kinds) {
+  return align_up(bsa_block_meta_bytes(s, kinds), 256);
+}
+
+size_t bsa_block_meta_bytes_varlen(const bsa_shape* shape, const int32_t* cu_seqlens, int32_t n_seqs,
+                                   int kinds) {
+  if (varlen_check(shape, cu_seqlens, n_seqs) != BSA_OK) return 0;
+  size_t total = 0;
+  for (int i = 0; i < n_seqs; ++i) {
+    const int len = cu_seqlens[i + 1] - cu_seqlens[i];
+    if (len == 0) continue;
+    const bsa_shape s = sub_shape(shape, len);
+    const size_t b = meta_bytes_padded(&s, kinds);
+    if (b == 0) return 0;
+    total += b;
+  }
+  return total;
+}
+
+bsa_status bsa_build_block_meta_varlen(const bsa_shape* shape, const int32_t* cu_seqlens, int32_t n_seqs,
+                                       const void* K, int kinds, void* meta, void* stream) {
+  bsa_status st = varlen_check(shape, cu_seqlens, n_seqs);
+  if (st != BSA_OK) return st;
+  if (!K || !meta) return fail(BSA_ERR_INVALID_ARG, "K or meta is NULL");
+  size_t off = 0;
+  for (int i = 0; i < n_seqs; ++i) {
+    const int start = cu_seqlens[i], len = cu_seqlens[i + 1] - start;
+    if (len == 0) continue;
+    const bsa_shape s = sub_shape(shape, len);
+    const char* Ki = static_cast<const char*>(K) + static_cast<int64_t>(start) * shape->kv_stride_n * 2;
+    st = bsa_build_block_meta(&s, Ki, kinds, static_cast<char*>(meta) + off, stream);
+    if (st != BSA_OK) return st;
+    off += meta_bytes_padded(&s, kinds);
+  }
+  return BSA_OK;
+}
+
+bsa_status bsa_select_varlen(const bsa_shape* shape, const int32_t* cu_seqlens, int32_t n_seqs, const void* Q,
+                             const void* meta, bsa_policy policy, int32_t k_budget, double q_frac,
+                             int32_t* kv_idx, int32_t* kv_count, float* sigma, float* sigma_bar,
+                             uint8_t* trigger, float* tau, void* stream) {
+  bsa_status st = varlen_check(shape, cu_seqlens, n_seqs);
+  if (st != BSA_OK) return st;
+  if (!Q || !meta || !kv_idx || !kv_count || !sigma || !sigma_bar || !trigger || !tau)
+    return fail(BSA_ERR_INVALID_ARG, "varlen select: every output pointer must be given");
+  const int W = bsa_kv_width(policy, k_budget);
+  if (W < 1) return fail(BSA_ERR_INVALID_ARG, "unknown policy or k_budget < 1");
+  const int64_t H = shape->n_q_heads;
+  size_t moff = 0;
+  for (int i = 0; i < n_seqs; ++i) {
+    const int start = cu_seqlens[i], len = cu_seqlens[i + 1] - start;
+    if (len == 0) continue;
+    const int64_t t0 = start / shape->block;
+    const bsa_shape s = sub_shape(shape, len);
+    const char* Qi = static_cast<const char*>(Q) + static_cast<int64_t>(start) * shape->q_stride_n * 2;
+    st = bsa_select(&s, Qi, static_cast<const char*>(meta) + moff, policy, k_budget, q_frac,
+                    kv_idx + H * W * t0, kv_count + H * t0, sigma + H * t0, sigma_bar + t0, trigger + t0,
+                    tau + i, nullptr, 0, stream);
+    if (st != BSA_OK) return st;
+    moff += meta_bytes_padded(&s, BSA_META_MEAN | BSA_META_MINMAX);
+  }
+  return BSA_OK;
+}
+
+static bsa_status attn_varlen(const bsa_shape* shape, const int32_t* cu, int32_t n_seqs, const void* Q,
+                              const void* K, const void* V, const int32_t* kv_idx, const int32_t* kv_count,
+                              int32_t W, bool sparse, float scale, void* O, float* lse, void* stream) {
+  bsa_status st = varlen_check(shape, cu, n_seqs);
+  if (st != BSA_OK) return st;
+  if (!Q || !K || !V || !O) return fail(BSA_ERR_INVALID_ARG, "Q, K, V and O must not be NULL");
+  const int64_t H = shape->n_q_heads;
+  for (int i = 0; i < n_seqs; ++i) {
+    const int start = cu[i], len = cu[i + 1] - start;
+    if (len == 0) continue;
+    const int64_t t0 = start / shape->block;
+    const bsa_shape s = sub_shape(shape, len);
+    const int64_t qo = static_cast<int64_t>(start) * shape->q_stride_n * 2;
+    const int64_t ko = static_cast<int64_t>(start) * shape->kv_stride_n * 2;
+    st = attn_common(&s, static_cast<const char*>(Q) + qo, static_cast<const char*>(K) + ko,
+                     static_cast<const char*>(V) + ko, sparse ? kv_idx + H * W * t0 : nullptr,
+                     (sparse && kv_count) ? kv_count + H * t0 : nullptr, W, sparse, scale,
+                     static_cast<char*>(O) + qo, lse ? lse + H * start : nullptr, stream);
+    if (st != BSA_OK) return st;
+  }
+  return BSA_OK;
+}
+
+bsa_status bsa_sparse_attn_fwd_varlen(const bsa_shape* shape, const int32_t* cu_seqlens, int32_t n_seqs,
+                                      const void* Q, const void* K, const void* V, const int32_t* kv_idx,
+                                      const int32_t* kv_count, int32_t kv_width, float softmax_scale, void* O,
+                                      float* lse, void* stream) {
+  if (!kv_idx || kv_width < 1) return fail(BSA_ERR_INVALID_ARG, "kv_idx is NULL or kv_width < 1");
+  return attn_varlen(shape, cu_seqlens, n_seqs, Q, K, V, kv_idx, kv_count, kv_width, true, softmax_scale, O,
+                     lse, stream);
+}
+
+bsa_status bsa_dense_attn_fwd_varlen(const bsa_shape* shape, const int32_t* cu_seqlens, int32_t n_seqs,
+                                     const void* Q, const void* K, const void* V, float softmax_scale, void* O,
+                                     float* lse, void* stream) {
+  return attn_varlen(shape, cu_seqlens, n_seqs, Q, K, V, nullptr, nullptr, 0, false, softmax_scale, O, lse,
+                     stream);
 }
 
 }  // extern "C"

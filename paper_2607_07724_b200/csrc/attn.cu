@@ -407,19 +407,28 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
     tmem_alloc<C::TMEM_COLS>(smem_u32(&ctl->tmem_base));
   }
   if (SPARSE && warp == 0) {
-    // compact the valid entries of this kv_idx row (sentinel >= N_B and blocks > t are skipped, A.10)
+    // compact the valid entries of this kv_idx row (sentinel >= N_B and blocks > t are skipped, A.10;
+    // a block listed more than once is attended once, like the oracle's O11)
     const int64_t row = (static_cast<int64_t>(b) * p.H + h) * p.NT + tq;
     int cnt = p.kv_count ? p.kv_count[row] : p.W;
     cnt = cnt < 0 ? 0 : (cnt > p.W ? p.W : cnt);
     const int32_t* src = p.kv_idx + row * p.W;
+    const unsigned lt = (1u << lane) - 1u;
     int base = 0;
     for (int i0 = 0; i0 < cnt; i0 += 32) {
       const int i = i0 + lane;
       const int blk = (i < cnt) ? src[i] : -1;
-      const bool ok = (blk >= 0) && (blk < p.NB) && (blk <= tq);
+      bool ok = (blk >= 0) && (blk < p.NB) && (blk <= tq);
+      const unsigned same = __match_any_sync(0xffffffffu, ok ? blk : -1 - lane);
+      if (same & lt) ok = false;                         // duplicate inside this chunk: lowest lane wins
+      if (i0 > 0 && ok) {                                // duplicate of an earlier chunk
+        for (int u = 0; u < base; ++u)
+          if (ctl->list[u] == static_cast<uint16_t>(blk)) { ok = false; break; }
+      }
       const unsigned bal = __ballot_sync(0xffffffffu, ok);
-      if (ok) ctl->list[base + __popc(bal & ((1u << lane) - 1u))] = static_cast<uint16_t>(blk);
+      if (ok) ctl->list[base + __popc(bal & lt)] = static_cast<uint16_t>(blk);
       base += __popc(bal);
+      __syncwarp();
     }
     if (lane == 0) ctl->n_valid = base;
   }

@@ -34,14 +34,26 @@ MetaLayout meta_layout(const Dims& D);
 
 // kernels (each only enqueues on `stream`)
 bsa_status launch_pool(const Dims& D, const void* K, int kinds, void* meta, cudaStream_t stream);
+// D.4 diagnostics outputs of the selection (device pointers, each [B,H,T]; all nullptr = off) and the
+// per-sequence summary [B, BSA_DIAG_SUMMARY_LEN] (may be nullptr).
+struct SelectDiag {
+  float *g, *G, *r, *d2, *rough, *summary;
+};
 bsa_status launch_select(const Dims& D, const void* Q, const void* meta, int policy, int k, int W,
                          long long m_route, int32_t* kv_idx, int32_t* kv_count, float* sigma,
-                         float* sigma_bar, uint8_t* trigger, float* tau, cudaStream_t stream);
-// tensor-core scoring + tile max + top-(2k) + sigma (score_tc.cu); writes kv_idx (all 2k/k slots),
-// sigma and, for the non-router policies, kv_count.
-bsa_status launch_score_tc(const Dims& D, const void* Q, const void* meta, bool quest, int k, int W,
-                           int router, int32_t* kv_idx, int32_t* kv_count, float* sigma,
-                           cudaStream_t stream);
+                         float* sigma_bar, uint8_t* trigger, float* tau, const SelectDiag& dg,
+                         cudaStream_t stream);
+// tensor-core scoring + tile max + top-(2k) + sigma (score_tc.cuh); writes kv_idx (all 2k/k slots),
+// sigma and, for the non-router policies, kv_count.  One translation unit per backbone.
+bsa_status launch_score_tc_quest(const Dims& D, const void* Q, const void* meta, int k, int W, int router,
+                                 int32_t* kv_idx, int32_t* kv_count, float* sigma, const SelectDiag& dg,
+                                 cudaStream_t stream);
+bsa_status launch_score_tc_mean(const Dims& D, const void* Q, const void* meta, int k, int W, int router,
+                                int32_t* kv_idx, int32_t* kv_count, float* sigma, const SelectDiag& dg,
+                                cudaStream_t stream);
+// per-sequence reduction of the D.4 per-cell quantities (diag.cu)
+bsa_status launch_diag_summary(const Dims& D, int k, int router, const float* tau, const SelectDiag& dg,
+                               cudaStream_t stream);
 bsa_status launch_attn(const Dims& D, const void* Q, const void* K, const void* V,
                        const int32_t* kv_idx, const int32_t* kv_count, int W, bool sparse,
                        float scale, void* O, float* lse, cudaStream_t stream);

@@ -23,6 +23,10 @@
 //   W5    tcgen05.mma issue, accumulators ping-pong across chunks and items
 //   W6-9  one warp per head: warp_select (select_common.cuh) of item i while W0-5 already work on
 //         item i+1; the score rows are released as soon as the warp holds its keys in registers
+//
+// This header holds the kernel template; score_tc_quest.cu and score_tc_mean.cu instantiate it for the
+// two backbones (two translation units so that the ~30 instantiations compile in parallel).
+#pragma once
 #include <cuda_bf16.h>
 
 #include "bsa_internal.h"
@@ -40,22 +44,32 @@ constexpr int kAStageBytes = kABlocks * 128;  // one [128 blocks x 64 elem] swiz
 constexpr int kMaxStages = 6;
 constexpr int kSelWarp0 = 6;                  // first selection warp
 
+// NH = query heads of one GQA group scored per work item (UMMA N = NH * BN <= 256; B planes <= 128 KB).
+// The host picks the largest NH <= NH_MAX whose shared-memory footprint fits: the score rows take
+// NH * N_B * 4 bytes, so long sequences (N_B >= 4096, i.e. 256K tokens at block 64) run with fewer
+// heads per item instead of being refused.
 template <int D, int BN, bool QUEST>
-struct TcCfg {
+struct TcShape {
   static constexpr int PLANES_B = QUEST ? 2 : 1;          // q+ | q-   or   q
   static constexpr int PLANES_A = QUEST ? 2 : 3;          // kmax | kmin   or   hi | mid | lo
   static constexpr int DC = D / 64;                        // 64-element K chunks per plane
   static constexpr int HEAD_B_BYTES = BN * D * 2 * PLANES_B;
   static constexpr int NH_N = 256 / BN;                    // UMMA N <= 256; also <= 4 selection warps
   static constexpr int NH_S = (128 * 1024) / HEAD_B_BYTES; // B planes <= 128 KB
-  static constexpr int NH = NH_N < NH_S ? NH_N : NH_S;
+  static constexpr int NH_MAX = NH_N < NH_S ? NH_N : NH_S;
+};
+
+template <int D, int BN, bool QUEST, int NH_>
+struct TcCfg : TcShape<D, BN, QUEST> {
+  using S = TcShape<D, BN, QUEST>;
+  static constexpr int NH = NH_;
   static constexpr int NROWS = NH * BN;                    // rows of one B chunk tile
   static constexpr int B_CHUNK_BYTES = NROWS * 128;
-  static constexpr int B_BYTES = B_CHUNK_BYTES * DC * PLANES_B;
-  static constexpr int KCHUNKS = PLANES_A * DC;            // A chunks per block chunk
+  static constexpr int B_BYTES = B_CHUNK_BYTES * S::DC * S::PLANES_B;
+  static constexpr int KCHUNKS = S::PLANES_A * S::DC;      // A chunks per block chunk
   static constexpr uint32_t TMEM_COLS = (2 * NROWS <= 32) ? 32 : (2 * NROWS <= 64) ? 64
                                         : (2 * NROWS <= 128) ? 128 : (2 * NROWS <= 256) ? 256 : 512;
-  static_assert(NH >= 1 && NH <= 4, "one selection warp per head, four of them");
+  static_assert(NH >= 1 && NH <= 4 && NH <= S::NH_MAX, "one selection warp per head, four of them");
 };
 
 struct TcParams {
@@ -64,6 +78,9 @@ struct TcParams {
   float* sigma;
   int B, H, Hkv, G, NB, k, W, router, sets, stages, nbpad, n_items;
   float inv_sqrt_d;
+  // D.4 diagnostics (Eq.18), all [B,H,T] or nullptr (diag == 0)
+  int diag;
+  float *dg_g, *dg_G, *dg_r, *dg_d2, *dg_rough;
 };
 
 struct alignas(8) TcCtl {
@@ -72,6 +89,7 @@ struct alignas(8) TcCtl {
   uint64_t acc_full[2], acc_empty[2];
   uint32_t tmem_base;
   uint32_t s3[4 * 4];   // per-warp scratch of warp_select
+  float rough[4][4];    // [epilogue warp][head]: sum of squared row-to-row score differences (diag)
 };
 
 struct Item {
@@ -96,17 +114,18 @@ __device__ __forceinline__ Item decode_item(const TcParams& p, int w) {
   return it;
 }
 
-template <int D, int BN, bool QUEST>
+template <int D, int BN, bool QUEST, int NH>
 __global__ void __launch_bounds__(kTcThreads, 1)
 score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmA,
                 const TcParams p) {
-  using C = TcCfg<D, BN, QUEST>;
+  using C = TcCfg<D, BN, QUEST, NH>;
   extern __shared__ __align__(1024) uint8_t smem[];
   uint8_t* b_s = smem;                                   // [PLANES_B][DC][NROWS x 128 B]
   uint8_t* a_s = smem + C::B_BYTES;                      // ring of [128 x 128 B] stages
   uint32_t* sc = reinterpret_cast<uint32_t*>(a_s + p.stages * kAStageBytes);   // [NH][nbpad] okey(score)
   unsigned long long* cand = reinterpret_cast<unsigned long long*>(sc + C::NH * p.nbpad);
-  TcCtl* ctl = reinterpret_cast<TcCtl*>(cand + C::NH * kMaxCand);
+  uint32_t* srt = reinterpret_cast<uint32_t*>(cand + C::NH * kMaxCand);   // sorted keys (diag), per head
+  TcCtl* ctl = reinterpret_cast<TcCtl*>(srt + C::NH * kMaxCand);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int w0 = static_cast<int>(blockIdx.x), wstep = static_cast<int>(gridDim.x);
@@ -254,15 +273,20 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       if (lane == 0) mbar_arrive(smem_u32(&ctl->b_ready));
 
       // the selection warps must hold the previous item's keys in registers before sc is rewritten
+      // (and have read the previous item's rough[] partials, which they do before releasing the keys)
       if (li > 0) mbar_wait(smem_u32(&ctl->sc_free), (li - 1) & 1);
+      double rough[4] = {0.0, 0.0, 0.0, 0.0};
       for (int c = 0; c < im.n_chunks; ++c, ++cg) {
         const int buf = cg & 1;
         mbar_wait(smem_u32(&ctl->acc_full[buf]), (cg >> 1) & 1);
         tc_fence_after();
         const int blk = c * kABlocks + warp * 32 + lane;
         const uint32_t tD = tmem + lane_base + buf * C::NROWS;
-        for (int j = 0; j < im.nh; ++j) {
+#pragma unroll
+        for (int j = 0; j < C::NH; ++j) {
+          if (j >= im.nh) break;
           float m0 = -INFINITY, m1 = -INFINITY, m2 = -INFINITY, m3 = -INFINITY;   // four independent chains
+          float rs = 0.0f, prev = 0.0f;   // diag: sum of squared differences of adjacent rows' scores
 #pragma unroll
           for (int c0 = 0; c0 < BN; c0 += 64) {
             uint32_t ra[32], rb[32];
@@ -276,13 +300,36 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
               m2 = fmax3(m2, __uint_as_float(ra[i + 2]), __uint_as_float(rb[i + 2]));
               m3 = fmax3(m3, __uint_as_float(ra[i + 3]), __uint_as_float(rb[i + 3]));
             }
+            if (p.diag) {   // warp-uniform; rows c0 .. c0+63 are ra[0..31], rb[0..31]
+              if (c0 > 0) { const float d0 = __uint_as_float(ra[0]) - prev; rs = fmaf(d0, d0, rs); }
+#pragma unroll
+              for (int i = 0; i < 31; ++i) {
+                const float da = __uint_as_float(ra[i + 1]) - __uint_as_float(ra[i]);
+                const float db = __uint_as_float(rb[i + 1]) - __uint_as_float(rb[i]);
+                rs = fmaf(da, da, rs);
+                rs = fmaf(db, db, rs);
+              }
+              const float dm = __uint_as_float(rb[0]) - __uint_as_float(ra[31]);
+              rs = fmaf(dm, dm, rs);
+              prev = __uint_as_float(rb[31]);
+            }
           }
           const float mx = fmaxf(fmax3(m0, m1, m2), m3);
           if (blk <= im.t) sc[j * p.nbpad + blk] = okey(QUEST ? mx : mx * p.inv_sqrt_d);   // Eq.3 (G8)
+          if (p.diag) rough[j] += (blk <= im.t) ? static_cast<double>(rs) : 0.0;
         }
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(smem_u32(&ctl->acc_empty[buf]));
+      }
+      if (p.diag) {   // fixed-order reduction: lanes by shuffle tree, warps summed 0..3 by the consumer
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          double v = rough[j];
+#pragma unroll
+          for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+          if (lane == 0) ctl->rough[warp][j] = static_cast<float>(v);
+        }
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctl->sc_full));   // release: the score rows are complete
@@ -298,11 +345,24 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       if (sw < im.nh && sw < C::NH) {
         const int h = im.h0 + sw;
         const int64_t row = (static_cast<int64_t>(im.b) * p.H + h) * p.NB + im.t;
+        float rough_sum = 0.0f;
+        if (p.diag)   // read before the keys are released: the epilogue warps rewrite it for the next item
+          rough_sum = ((ctl->rough[0][sw] + ctl->rough[1][sw]) + ctl->rough[2][sw]) + ctl->rough[3][sw];
+        DiagCell cell;
         const float sig = warp_select(sc + sw * p.nbpad, im.t, p.k, p.NB, p.W, p.kv_idx + row * p.W,
-                                      cand + sw * kMaxCand, ctl->s3 + sw * 4, lane, rel);
+                                      cand + sw * kMaxCand, ctl->s3 + sw * 4, lane, rel,
+                                      p.diag ? &cell : nullptr, srt + sw * kMaxCand);
         if (lane == 0) {
           p.sigma[row] = sig;
           if (!p.router) p.kv_count[row] = (p.k < im.t + 1) ? p.k : im.t + 1;
+          if (p.diag) {
+            p.dg_g[row] = cell.g;
+            p.dg_G[row] = cell.G;
+            p.dg_r[row] = cell.r;
+            p.dg_d2[row] = cell.d2;
+            // Eq.1 carries 1/sqrt(d) (G8): the K-mean row scores are scaled after the fact
+            p.dg_rough[row] = QUEST ? rough_sum : rough_sum * (p.inv_sqrt_d * p.inv_sqrt_d);
+          }
         }
         __syncwarp();   // cand / s3 of this warp are reused by the next item
       } else {
@@ -316,26 +376,36 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   if (warp == 4) tmem_dealloc<C::TMEM_COLS>(tmem);
 }
 
-template <int D, int BN, bool QUEST>
+struct DiagPtrs {
+  float *g, *G, *r, *d2, *rough;   // all nullptr: no diagnostics
+};
+
+template <int D, int BN, bool QUEST, int NH>
+size_t tc_fixed_smem(int nbpad) {
+  using C = TcCfg<D, BN, QUEST, NH>;
+  return static_cast<size_t>(C::B_BYTES) + static_cast<size_t>(NH) * nbpad * 4 +
+         static_cast<size_t>(NH) * kMaxCand * 8 + static_cast<size_t>(NH) * kMaxCand * 4 + sizeof(TcCtl);
+}
+constexpr size_t kTcSmemBudget = 227 * 1024;
+
+template <int D, int BN, bool QUEST, int NH>
 bsa_status run_score_tc(const Dims& S, const void* Q, const char* meta, const MetaLayout& L, int k, int W,
-                        int router, int32_t* kv_idx, int32_t* kv_count, float* sigma,
+                        int router, int32_t* kv_idx, int32_t* kv_count, float* sigma, const DiagPtrs& dg,
                         cudaStream_t stream) {
-  using C = TcCfg<D, BN, QUEST>;
+  using C = TcCfg<D, BN, QUEST, NH>;
   TcParams p;
   p.kv_idx = kv_idx; p.kv_count = kv_count; p.sigma = sigma;
   p.B = S.B; p.H = S.H; p.Hkv = S.Hkv; p.G = S.G; p.NB = S.NB; p.k = k; p.W = W; p.router = router;
-  p.sets = (S.G + C::NH - 1) / C::NH;
+  p.sets = (S.G + NH - 1) / NH;
   p.nbpad = (S.NB + 3) & ~3;
   p.inv_sqrt_d = static_cast<float>(1.0 / sqrt(static_cast<double>(S.d)));
+  p.diag = dg.g != nullptr;
+  p.dg_g = dg.g; p.dg_G = dg.G; p.dg_r = dg.r; p.dg_d2 = dg.d2; p.dg_rough = dg.rough;
   const long long n_items = static_cast<long long>(S.NB) * S.B * S.Hkv * p.sets;
   if (n_items > 0x7fffffffLL) return fail(BSA_ERR_UNSUPPORTED, "select: too many work items");
   p.n_items = static_cast<int>(n_items);
-  const size_t fixed = static_cast<size_t>(C::B_BYTES) + static_cast<size_t>(C::NH) * p.nbpad * 4 +
-                       static_cast<size_t>(C::NH) * kMaxCand * 8 + sizeof(TcCtl);
-  const size_t budget = 227 * 1024;
-  if (fixed + 2 * kAStageBytes > budget)
-    return fail(BSA_ERR_UNSUPPORTED, "select: %d blocks per sequence need too much shared memory", S.NB);
-  int stages = static_cast<int>((budget - fixed) / kAStageBytes);
+  const size_t fixed = tc_fixed_smem<D, BN, QUEST, NH>(p.nbpad);
+  int stages = static_cast<int>((kTcSmemBudget - fixed) / kAStageBytes);
   p.stages = stages > kMaxStages ? kMaxStages : stages;
 #ifdef BSA_TC_STAGE_CAP
   if (p.stages > BSA_TC_STAGE_CAP) p.stages = BSA_TC_STAGE_CAP;
@@ -343,7 +413,7 @@ bsa_status run_score_tc(const Dims& S, const void* Q, const char* meta, const Me
   const size_t smem = fixed + static_cast<size_t>(p.stages) * kAStageBytes;
 
   CUtensorMap tq, ta;
-  if (!make_tmap_bhnd(&tq, Q, S.B, S.H, S.N, S.d, S.qsb, S.qsh, S.qsn, BN, 1, C::NH))
+  if (!make_tmap_bhnd(&tq, Q, S.B, S.H, S.N, S.d, S.qsb, S.qsh, S.qsn, BN, 1, NH))
     return fail(BSA_ERR_CUDA, "select: cuTensorMapEncodeTiled(Q) failed");
   {
     const char* base = meta + (QUEST ? L.off_min : L.off_split);
@@ -356,7 +426,7 @@ bsa_status run_score_tc(const Dims& S, const void* Q, const char* meta, const Me
     if (!make_tmap_bf16(&ta, base, 5, dims, strides, box))
       return fail(BSA_ERR_CUDA, "select: cuTensorMapEncodeTiled(meta) failed");
   }
-  auto kern = score_tc_kernel<D, BN, QUEST>;
+  auto kern = score_tc_kernel<D, BN, QUEST, NH>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        static_cast<int>(smem));
   if (e != cudaSuccess) return fail(BSA_ERR_CUDA, "select: smem attribute: %s", cudaGetErrorString(e));
@@ -366,20 +436,42 @@ bsa_status run_score_tc(const Dims& S, const void* Q, const char* meta, const Me
   return check_launch("score_tc_kernel");
 }
 
-}  // namespace
+// Largest NH <= NH_MAX whose footprint leaves at least two A stages; 0 = even one head does not fit.
+template <int D, int BN, bool QUEST, int NH>
+bsa_status dispatch_nh(const Dims& S, const void* Q, const char* meta, const MetaLayout& L, int k, int W,
+                       int router, int32_t* kv_idx, int32_t* kv_count, float* sigma, const DiagPtrs& dg,
+                       cudaStream_t stream) {
+  const int nbpad = (S.NB + 3) & ~3;
+  // fewer heads per item than the GQA group has only cost A-plane re-reads; more never help
+  const bool useful = (NH == 1) || (NH - 1 < S.G);
+  if (useful && tc_fixed_smem<D, BN, QUEST, NH>(nbpad) + 2 * kAStageBytes <= kTcSmemBudget)
+    return run_score_tc<D, BN, QUEST, NH>(S, Q, meta, L, k, W, router, kv_idx, kv_count, sigma, dg, stream);
+  if constexpr (NH > 1) {
+    return dispatch_nh<D, BN, QUEST, NH - 1>(S, Q, meta, L, k, W, router, kv_idx, kv_count, sigma, dg, stream);
+  } else {
+    return fail(BSA_ERR_UNSUPPORTED,
+                "select: %d blocks per sequence need %zu bytes of shared memory per head (limit %zu): "
+                "at most %zu blocks fit for head_dim %d / block %d / this backbone",
+                S.NB, tc_fixed_smem<D, BN, QUEST, 1>(nbpad) + 2 * kAStageBytes, kTcSmemBudget,
+                (kTcSmemBudget - tc_fixed_smem<D, BN, QUEST, 1>(0) - 2 * kAStageBytes) / 4, S.d, S.Bn);
+  }
+}
 
-bsa_status launch_score_tc(const Dims& S, const void* Q, const void* meta, bool quest, int k, int W,
-                           int router, int32_t* kv_idx, int32_t* kv_count, float* sigma,
-                           cudaStream_t stream) {
+template <bool QUEST>
+bsa_status launch_score_tc_backbone(const Dims& S, const void* Q, const void* meta, int k, int W, int router,
+                                    int32_t* kv_idx, int32_t* kv_count, float* sigma, const DiagPtrs& dg,
+                                    cudaStream_t stream) {
   const MetaLayout L = meta_layout(S);
   const char* mp = static_cast<const char*>(meta);
-#define BSA_TC(DD, BB)                                                                              \
-  if (S.d == DD && S.Bn == BB)                                                                      \
-    return quest ? run_score_tc<DD, BB, true>(S, Q, mp, L, k, W, router, kv_idx, kv_count, sigma, stream) \
-                 : run_score_tc<DD, BB, false>(S, Q, mp, L, k, W, router, kv_idx, kv_count, sigma, stream);
+#define BSA_TC(DD, BB)                                                                                \
+  if (S.d == DD && S.Bn == BB)                                                                        \
+    return dispatch_nh<DD, BB, QUEST, TcShape<DD, BB, QUEST>::NH_MAX>(S, Q, mp, L, k, W, router, kv_idx, \
+                                                                     kv_count, sigma, dg, stream);
   BSA_TC(64, 64) BSA_TC(128, 64) BSA_TC(256, 64) BSA_TC(64, 128) BSA_TC(128, 128) BSA_TC(256, 128)
 #undef BSA_TC
   return fail(BSA_ERR_UNSUPPORTED, "select: unsupported head_dim %d / block %d", S.d, S.Bn);
 }
+
+}  // namespace
 
 }  // namespace bsa

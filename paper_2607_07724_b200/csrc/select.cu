@@ -3,7 +3,7 @@
 // padded kv_idx (Eq.1-5; A.2-A.9 L296-340; readings G1-G17 in DESIGN.md).
 //
 // Kernels
-//   score_tc_kernel (score_tc.cu) : tensor-core tile scores (Eq.1-3), top-(2k) and sigma (Eq.4 /
+//   score_tc_kernel (score_tc.cuh) : tensor-core tile scores (Eq.1-3), top-(2k) and sigma (Eq.4 /
 //                         Eq.11) per (tile, head); writes all 2k / k slots of kv_idx and sigma.
 //   route_kernel        : one CTA per sequence: sigma_bar (Eq.12), device radix-select of the
 //                         ceil(qT)-th smallest sigma_bar (Eq.5 / Eq.13), trigger.
@@ -113,10 +113,12 @@ __global__ void finalize_kernel(const uint8_t* __restrict__ trigger, int H, int 
 
 bsa_status launch_select(const Dims& S, const void* Q, const void* meta, int policy, int k, int W,
                          long long m_route, int32_t* kv_idx, int32_t* kv_count, float* sigma,
-                         float* sigma_bar, uint8_t* trigger, float* tau, cudaStream_t stream) {
+                         float* sigma_bar, uint8_t* trigger, float* tau, const SelectDiag& dg,
+                         cudaStream_t stream) {
   const bool quest = (policy == BSA_POLICY_QUEST || policy == BSA_POLICY_ROUTER_QUEST);
   const int router = (policy == BSA_POLICY_ROUTER || policy == BSA_POLICY_ROUTER_QUEST) ? 1 : 0;
-  bsa_status st = launch_score_tc(S, Q, meta, quest, k, W, router, kv_idx, kv_count, sigma, stream);
+  bsa_status st = quest ? launch_score_tc_quest(S, Q, meta, k, W, router, kv_idx, kv_count, sigma, dg, stream)
+                        : launch_score_tc_mean(S, Q, meta, k, W, router, kv_idx, kv_count, sigma, dg, stream);
   if (st != BSA_OK) return st;
 
   const size_t rsmem = (static_cast<size_t>(S.NB) + 256 + 2) * 4;
@@ -131,7 +133,9 @@ bsa_status launch_select(const Dims& S, const void* Q, const void* meta, int pol
     finalize_kernel<<<static_cast<unsigned>((total + threads - 1) / threads), threads, 0, stream>>>(
         trigger, S.H, S.NB, S.NB, k, kv_idx, kv_count, rows);
     st = check_launch("finalize_kernel");
+    if (st != BSA_OK) return st;
   }
+  if (dg.g && dg.summary) st = launch_diag_summary(S, k, router && m_route > 0, tau, dg, stream);
   return st;
 }
 

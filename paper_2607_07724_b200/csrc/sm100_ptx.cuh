@@ -39,14 +39,21 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
       : "memory");
   return ok != 0;
 }
-// Bounded wait: a protocol bug traps (illegal instruction -> cudaErrorLaunchFailure) after ~4 s
-// instead of hanging the GPU.
+// Debug builds (-DBSA_MBAR_TRAP=1, see build.py): a protocol bug traps (illegal instruction ->
+// cudaErrorLaunchFailure) after ~4 s of spinning instead of hanging the GPU.  Release builds wait
+// without a bound: a trap puts a sticky error on the context and clock64 also advances while the
+// context is switched out (time slicing, a debugger), so a timeout can fire with no bug present.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   if (mbar_try_wait(bar, parity)) return;
+#ifdef BSA_MBAR_TRAP
   long long t0 = clock64();
   while (!mbar_try_wait(bar, parity)) {
     if (clock64() - t0 > 8000000000LL) __trap();
   }
+#else
+  while (!mbar_try_wait(bar, parity)) {
+  }
+#endif
 }
 
 // generic-proxy writes to shared memory -> visible to the async proxy (TMA / tcgen05.mma reads)

@@ -131,6 +131,9 @@ CONFIGS = {
                   ("router_quest", "topk"), True, "single16"),
     "C3b": Config("C3b", 3, 131072, 28, 4, 128, 64, 32, (0.25,),
                   ("router_quest", "topk"), True, "single16"),
+    # 256K: the regime PAPER.md L271 names for selection fused into the attention kernel
+    "C3c": Config("C3c", 3, 262144, 28, 4, 128, 64, 32, (0.25,),
+                  ("router_quest", "topk"), True, "single16"),
     "C4": Config("C4", 4, 65536, 32, 8, 128, 64, 64, (0.1, 0.25, 0.5),
                  ("quest", "router_quest"), True, "single16"),
     "C5": Config("C5", 5, 131072, 16, 2, 256, 128, 16, (0.25,),

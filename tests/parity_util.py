@@ -6,9 +6,16 @@ from __future__ import annotations
 import numpy as np
 
 TIE_REL = 1e-5          # north_star: fp32 block scores closer than this (relative) may swap
-SIGMA_TOL = 1e-4        # sigma divides two small score differences
-SIGMA_BAR_BAND = 2e-4   # |sigma_bar - tau| below which a trigger may flip: both sides are means of
-                        # sigmas that are each within SIGMA_TOL (logged, counted, never hidden)
+SIGMA_TOL = 1e-4        # sigma divides two small score differences (SURVEY 8(c) protocol item 1)
+SIGMA_BAR_TOL = 1e-5    # sigma_bar / tau: a mean of sigmas; measured max |diff| is logged per case
+SCORE_REL = 2e-6        # agreement of the GPU's tile scores (exact bf16 products, fp32 accumulation in the
+                        # tensor core's own order) with the oracle's correctly rounded ones: a fifth of
+                        # north_star's 1e-5 score band.  sigma = (a-b)/(c-b) amplifies a score error e by
+                        # <= 4 e / (c-b): where that first-order image exceeds the fixed tolerances above
+                        # (small denominators: few visible blocks, near-flat score lists) it is the bound.
+                        # The measured maximum of |dsigma| (c-b) / (4 scale) is logged per case.
+SIGMA_BAR_BAND = 1e-5   # a trigger may differ only on tiles with |sigma_bar - tau| <= 1e-5 (SURVEY 8(c)
+                        # protocol item 1); each such tile is logged with its gap, never hidden
 ATTN_MAX_ABS = 2e-2
 ATTN_MEAN_ABS = 2e-3
 
@@ -28,10 +35,36 @@ def bf16_to_f32(bits: np.ndarray) -> np.ndarray:
     return (bits.astype(np.uint32) << np.uint32(16)).view(np.float32)
 
 
+def sigma_amp(score_sorted: np.ndarray, tiles, k: int) -> np.ndarray:
+    """scale / den per (tile, head) from the ORACLE's sorted scores [n, H, 2k+1]: den = s~[f] - s~[k],
+    scale = max(|s~[f]|, |s~[k]|); 0 where sigma is 1 by convention (t + 1 <= k), inf where den == 0."""
+    ss = np.asarray(score_sorted, np.float64)
+    n, H, _ = ss.shape
+    amp = np.zeros((n, H))
+    for i, t in enumerate(tiles):
+        if t + 1 <= k:
+            continue
+        f = 1 if t == 0 else 2
+        den = ss[i, :, f] - ss[i, :, k]
+        scale = np.maximum(np.abs(ss[i, :, f]), np.abs(ss[i, :, k]))
+        with np.errstate(divide="ignore", invalid="ignore"):
+            amp[i] = np.where(den > 0, scale / den, np.inf)
+    return amp
+
+
+def sigma_tolerances(amp: np.ndarray):
+    """(tol_sigma [n, H], tol_sigma_bar [n]) from sigma_amp()."""
+    img = 4.0 * SCORE_REL * amp
+    return np.maximum(SIGMA_TOL, img), np.maximum(SIGMA_BAR_TOL, img.mean(axis=1))
+
+
 def compare_select(gpu: dict, orc: dict, n_blocks: int, k: int, log: list | None = None):
     """gpu: numpy arrays kv_idx [H,T,W], kv_count [H,T], sigma [H,T], sigma_bar [T], trigger [T], tau.
-    orc: oracle.select(..., want_scores=True) result.  Returns a dict of counters; raises on a
-    mismatch outside the tie bands."""
+    orc: oracle.select(..., want_scores=True) result.  Returns a dict of counters and the measured
+    maxima; raises on any mismatch outside the two bands north_star / SURVEY 8(c) allow:
+      * kv_idx rows differ only where the swapped blocks' ORACLE scores are within 1e-5 relative;
+      * trigger differs only on tiles with |sigma_bar - tau| <= 1e-5.
+    Every exception is appended to `log` as a record (kind, t, h, blocks, scores)."""
     log = log if log is not None else []
     H, T, W = orc["kv_idx"].shape
     ts = orc["tile_score"]                      # [T, H, NB]
@@ -43,13 +76,24 @@ def compare_select(gpu: dict, orc: dict, n_blocks: int, k: int, log: list | None
     for t in flip:
         gap = abs(float(orc["sigma_bar"][t]) - tau)
         assert gap <= SIGMA_BAR_BAND, f"trigger differs at tile {t}: sigma_bar-tau gap {gap:g}"
-        log.append(("trigger", int(t), gap))
+        log.append(dict(kind="trigger", t=int(t), gap=gap, sigma_bar_oracle=float(orc["sigma_bar"][t]),
+                        sigma_bar_gpu=float(gpu["sigma_bar"][t]), tau_oracle=float(tau),
+                        tau_gpu=float(gpu["tau"])))
     stats["trigger_flips"] = len(flip)
     flipped = np.zeros(T, bool)
     flipped[flip] = True
-    assert len(flip) <= max(2, T // 100), f"{len(flip)} trigger flips"
-    assert abs(float(gpu["tau"]) - tau) <= SIGMA_TOL, "tau"
-    np.testing.assert_allclose(gpu["sigma_bar"], orc["sigma_bar"], rtol=0, atol=SIGMA_TOL)
+    amp = sigma_amp(orc["score_sorted"], range(T), k)                      # [T, H]
+    tol_sig, tol_bar = sigma_tolerances(amp)
+    d_sig = np.abs(gpu["sigma"].astype(np.float64) - orc["sigma"])          # [H, T]
+    d_bar = np.abs(gpu["sigma_bar"].astype(np.float64) - orc["sigma_bar"])
+    stats["max_dtau"] = abs(float(gpu["tau"]) - tau)
+    stats["max_dsigma_bar"] = float(d_bar.max())
+    stats["max_dsigma"] = float(d_sig.max())
+    fin = np.isfinite(amp.T) & (amp.T > 0)
+    stats["max_score_rel_implied"] = float((d_sig[fin] / (4.0 * amp.T[fin])).max()) if fin.any() else 0.0
+    assert stats["max_dtau"] <= tol_bar.max(), f"tau {gpu['tau']} vs {tau}"
+    bad = d_bar > tol_bar
+    assert not bad.any(), f"sigma_bar differs at tiles {np.nonzero(bad)[0][:8]}: {d_bar[bad][:8]} > {tol_bar[bad][:8]}"
 
     # ---- kv_count: exact wherever the trigger agrees ----
     ok_t = ~flipped
@@ -57,41 +101,44 @@ def compare_select(gpu: dict, orc: dict, n_blocks: int, k: int, log: list | None
 
     # ---- kv_idx ----
     same = (gpu["kv_idx"] == orc["kv_idx"]).all(axis=2)          # [H, T]
-    sig_bad = np.abs(gpu["sigma"] - orc["sigma"]) > SIGMA_TOL
     for h, t in zip(*np.nonzero(~same)):
         if flipped[t]:
             continue
         cnt = int(orc["kv_count"][h, t])
         g_row, o_row = gpu["kv_idx"][h, t], orc["kv_idx"][h, t]
-        assert (g_row[cnt:] == n_blocks).all(), f"padding not sentinel at h={h} t={t}"
-        assert g_row[0] == 0 and (t == 0 or g_row[1] == t), f"forced blocks missing at h={h} t={t}"
-        gs, os_ = set(g_row[:cnt].tolist()), set(o_row[:cnt].tolist())
-        assert len(gs) == cnt and all(0 <= b <= t for b in gs), f"invalid blocks at h={h} t={t}"
-        sc = ts[t, h]
-        # every position where the rows differ must be a near-tie between the two blocks placed there
-        for gb, ob in zip(g_row[:cnt], o_row[:cnt]):
-            if gb != ob:
-                a, b = float(sc[gb]), float(sc[ob])
-                assert abs(a - b) <= TIE_REL * max(abs(a), abs(b)), \
-                    f"kv_idx differs outside the tie band at h={h} t={t}: blocks {gb},{ob} scores {a},{b}"
-        # set difference (cutoff swaps) must be near-ties with the boundary score
-        for blk in gs ^ os_:
-            bnd = float(sc[o_row[cnt - 1]])
-            a = float(sc[blk])
-            assert abs(a - bnd) <= TIE_REL * max(abs(a), abs(bnd)), \
-                f"selected set differs outside the tie band at h={h} t={t}: block {blk}"
+        rec = check_row(g_row, o_row, cnt, ts[t, h], int(t), n_blocks, f"h={h} t={t}")
         stats["tie_rows"] += 1
-        log.append(("kv_idx", int(h), int(t)))
-    # sigma: 1e-4 absolute, except rows whose cutoff is itself inside the tie band
-    for h, t in zip(*np.nonzero(sig_bad)):
-        ss = orc["score_sorted"][t, h]
-        f = 1 if t == 0 else 2
-        den = float(ss[f]) - float(ss[k])
-        scale = max(abs(float(ss[f])), abs(float(ss[k])))
-        assert den <= 100 * TIE_REL * scale, \
-            f"sigma differs at h={h} t={t}: {gpu['sigma'][h, t]} vs {orc['sigma'][h, t]} (den {den:g})"
-        log.append(("sigma", int(h), int(t)))
+        log.append(dict(kind="kv_idx", t=int(t), h=int(h), **rec))
+    # sigma: 1e-4 absolute, or the first-order image of a SCORE_REL score error where that is larger
+    bad = d_sig > tol_sig.T
+    assert not bad.any(), (f"sigma differs on {int(bad.sum())} rows, first (h,t)="
+                           f"{tuple(int(x[0]) for x in np.nonzero(bad))}: {d_sig[bad][:4]} > {tol_sig.T[bad][:4]}")
+    stats["sigma_rows_over_1e-4"] = int((d_sig > SIGMA_TOL).sum())
     return stats
+
+
+def check_row(g_row, o_row, cnt, sc, t, n_blocks, what):
+    """One kv_idx row of the GPU against the oracle's.  Bit-exact, or every block that sits at a
+    different position / in only one of the two sets has an ORACLE score within 1e-5 relative of the
+    block it displaced (north_star).  Returns the record for the tie log: the differing blocks and
+    their oracle scores."""
+    assert (g_row[cnt:] == n_blocks).all(), f"{what}: padding not sentinel"
+    assert g_row[0] == 0 and (t == 0 or g_row[1] == t), f"{what}: forced blocks missing"
+    gs, os_ = set(g_row[:cnt].tolist()), set(o_row[:cnt].tolist())
+    assert len(gs) == cnt and all(0 <= b <= t for b in gs), f"{what}: invalid blocks"
+    blocks, scores = [], []
+    for gb, ob in zip(g_row[:cnt], o_row[:cnt]):
+        if gb != ob:
+            a, b = float(sc[gb]), float(sc[ob])
+            assert abs(a - b) <= TIE_REL * max(abs(a), abs(b)), \
+                f"{what}: kv_idx differs outside the tie band: blocks {gb},{ob} scores {a},{b}"
+            blocks.append([int(gb), int(ob)])
+            scores.append([a, b])
+    for blk in gs ^ os_:
+        bnd, a = float(sc[o_row[cnt - 1]]), float(sc[blk])
+        assert abs(a - bnd) <= TIE_REL * max(abs(a), abs(bnd)), \
+            f"{what}: selected set differs outside the tie band: block {blk} score {a} boundary {bnd}"
+    return dict(blocks=blocks, scores=scores, set_diff=sorted(int(b) for b in gs ^ os_))
 
 
 def compare_attn(O_gpu_f32: np.ndarray, O_ref: np.ndarray, what: str = ""):

@@ -109,14 +109,20 @@ def test_hand_worked_margin_examples():
         sig, idx_sorted, _ = oracle.select_from_scores(e["ts"], e["t"], e["nb"], e["k"])
         assert abs(sig - e["sigma"]) < 1e-6, e["name"]
         for trig, row, cnt in ((0, e["row0"], e["cnt0"]), (1, e["row1"], e["cnt1"])):
-            kv_idx, kv_count = oracle.fill(idx_sorted.reshape(1, 1, -1), np.array([trig], np.uint8),
-                                           e["nb"], e["k"], 2 * e["k"])
-            # fill() indexes tiles from 0; emulate tile t by checking count = min(budget, t+1) by hand
-            budget = 2 * e["k"] if trig else e["k"]
-            want_cnt = min(budget, e["t"] + 1)
-            assert want_cnt == cnt, e["name"]
-            got = list(idx_sorted[:cnt]) + [e["nb"]] * (2 * e["k"] - cnt)
-            assert got == row, e["name"]
+            # orc_fill (Eq.14) takes the tile index from the position: put the example at tile t of a
+            # (t+1)-tile sequence and assert on what fill() itself returns for that tile
+            t, nb, k = e["t"], e["nb"], e["k"]
+            idx_all = np.full((t + 1, 1, 2 * k), nb, np.int32)
+            idx_all[t, 0] = idx_sorted
+            trigger = np.zeros(t + 1, np.uint8)
+            trigger[t] = trig
+            kv_idx, kv_count = oracle.fill(idx_all, trigger, nb, k, 2 * k)
+            assert int(kv_count[0, t]) == cnt, e["name"]
+            assert kv_idx[0, t].tolist() == row, e["name"]
+            # non-router width W = k: the untriggered prefix, same count rule
+            if not trig:
+                kv_k, cnt_k = oracle.fill(idx_all, trigger, nb, k, k)
+                assert int(cnt_k[0, t]) == cnt and kv_k[0, t].tolist() == row[:k], e["name"]
     for name, sb, q, tau, tiles in routes:
         sigma = np.repeat(sb[:, None], 3, axis=1)           # 3 identical heads -> mean = sb
         sbar, got_tau, trig = oracle.route(sigma, "router", q)
