@@ -194,10 +194,10 @@ def oracle_sample_ms(cfg, inp, policy: str, q_frac: float, stride: int = 16):
 
 def reference_stride(cfg, steps_total: int, cores: int) -> int:
     """Tile stride (a power of two) that keeps the whole reference run near 2-3 minutes: the oracle does
-    about 1.2e8 MAC/s per core (measured: C2 in full, 6e10 scoring + 7e10 attention MAC, 34 s on 16)."""
+    2.3e8 (C2 in full: 33 s on 16 cores) to 7e8 (128K samples) MAC/s per core; 4e8 is assumed."""
     work = cfg.n_blocks * (cfg.n_blocks + 1) / 2 * cfg.block * cfg.head_dim * cfg.n_q_heads * 4.0
     per_step_s = 150.0 / max(steps_total, 1)
-    need = work / (1.2e8 * max(cores, 1) * per_step_s)
+    need = work / (4e8 * max(cores, 1) * per_step_s)
     return int(min(512, max(1, 2 ** math.ceil(math.log2(max(need, 1))))))
 
 
@@ -600,7 +600,7 @@ def run_gpu(args):
     import oracle
     cores = oracle.max_threads()
     work = cfg.n_blocks * (cfg.n_blocks + 1) / 2 * cfg.block * cfg.head_dim * cfg.n_q_heads * 4.0
-    stride = int(min(512, max(1, 2 ** math.ceil(math.log2(max(work / (1.2e8 * cores * 25.0), 1))))))
+    stride = int(min(512, max(1, 2 ** math.ceil(math.log2(max(work / (4e8 * cores * 20.0), 1))))))
     cb = oracle_sample_ms(cfg, inp, args.policy, args.q_frac, stride)
     line["cpu_baseline"] = {"value": cb["value"], "unit": "ms", "cores": cores, "kind": "oracle",
                             "sample": cb["sample"], "measured_ms": cb["measured_ms"], "scale": cb["scale"],

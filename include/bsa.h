@@ -200,6 +200,25 @@ bsa_status bsa_dense_attn_fwd_varlen(const bsa_shape* shape, const int32_t* cu_s
                                      const void* Q, const void* K, const void* V, float softmax_scale, void* O,
                                      float* lse, void* stream);
 
+/*
+ * Per-row selection scattered into a per-tile block bitmap (section 4.5 item 1, L269: "A per-row
+ * scatter-into-bitmap kernel would close the rest of the gap without re-materialising the [B, H, M, N_B]
+ * keep tensor"; reading G18).  Every query row i of tile t ranks the visible blocks b <= t
+ * by its OWN row score (Eq.1 with BSA_POLICY_TOPK, Eq.2 with BSA_POLICY_QUEST; no tile max), blocks 0 and t
+ * forced on top (Eq.9), ties -> lower block index (G6), and keeps its first min(k_row, t+1) blocks; the
+ * tile's bitmap is the union over its rows and the whole tile attends the union.
+ *   bitmap   [B, Hq, Q_t, bsa_bitmap_words(shape)] uint32: bit (b % 32) of word (b / 32) = block b
+ *   kv_count [B, Hq, Q_t] int32: number of set bits (between min(k_row, t+1) and min(t+1, 2 + block (k_row-2)))
+ * Limits: 3 <= k_row <= 64.  bsa_sparse_attn_fwd_bitmap attends the set blocks of every row (bits above
+ * t are ignored; the block equal to t gets the causal mask); N_B <= 4096.
+ */
+size_t bsa_bitmap_words(const bsa_shape* shape);
+bsa_status bsa_select_rows_bitmap(const bsa_shape* shape, const void* Q, const void* meta, bsa_policy policy,
+                                  int32_t k_row, uint32_t* bitmap, int32_t* kv_count, void* stream);
+bsa_status bsa_sparse_attn_fwd_bitmap(const bsa_shape* shape, const void* Q, const void* K, const void* V,
+                                      const uint32_t* bitmap, float softmax_scale, void* O, float* lse,
+                                      void* stream);
+
 /* Thread-local, static storage; never NULL. */
 const char* bsa_last_error(void);
 

@@ -58,6 +58,8 @@ def _load():
         lib.orc_roughness.restype = None
         lib.orc_diag_summary.argtypes = [vp, vp, vp, vp, i64, i64, i64, i64, ci, ctypes.c_float, vp]
         lib.orc_diag_summary.restype = None
+        lib.orc_select_rows_bitmap.argtypes = [vp, vp, vp, vp, i64, i64, i64, i64, i64, ci, i64, vp, i64, vp, vp]
+        lib.orc_select_rows_bitmap.restype = None
         lib.orc_max_threads.restype = ci
         _lib = lib
     return _lib
@@ -246,3 +248,34 @@ def diag(Q, meta, block: int, policy: str, k: int, q_frac: float):
     router = policy in ("router", "router_quest") and tau >= 0
     summ, vec = diag_summary(cells["g"], cells["r"], cells["d2"], rough, k, block, router, tau)
     return dict(cells, rough=rough, summary=summ, summary_vec=vec, tau=tau)
+
+
+# ---- per-row selection scattered into a per-tile bitmap --------------------------------
+def select_rows_bitmap(Q, meta, block: int, policy: str, k_row: int, tiles=None):
+    """Returns (bitmap uint32 [n_tiles, H, ceil(N_B/32)], count int32 [n_tiles, H])."""
+    Q = _c(Q, np.uint16)
+    kmean, kmin, kmax = meta
+    H, N, d = Q.shape
+    NB = N // block
+    tiles = _c(np.arange(NB) if tiles is None else np.asarray(tiles), np.int64)
+    n = len(tiles)
+    bitmap = np.empty((n, H, (NB + 31) // 32), np.uint32)
+    count = np.empty((n, H), np.int32)
+    _load().orc_select_rows_bitmap(_p(Q), _p(_c(kmean, np.float32)), _p(_c(kmin, np.uint16)),
+                                   _p(_c(kmax, np.uint16)), H, kmean.shape[0], N, d, block, POLICIES[policy],
+                                   k_row, _p(tiles), n, _p(bitmap), _p(count))
+    return bitmap, count
+
+
+def bitmap_to_kv_idx(bitmap, n_blocks: int):
+    """[n, H, NBW] -> (kv_idx [H, n, width] ascending block lists padded with n_blocks, kv_count [H, n])."""
+    n, H, _ = bitmap.shape
+    bits = np.unpackbits(bitmap.view(np.uint8), axis=-1, bitorder="little")[..., :n_blocks]
+    cnt = bits.sum(-1).astype(np.int32)
+    W = int(cnt.max()) if cnt.size else 1
+    kv = np.full((H, n, max(W, 1)), n_blocks, np.int32)
+    for i in range(n):
+        for h in range(H):
+            idx = np.nonzero(bits[i, h])[0]
+            kv[h, i, :len(idx)] = idx
+    return kv, np.ascontiguousarray(cnt.T)

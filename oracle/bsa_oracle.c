@@ -18,6 +18,8 @@
  * k_budget >= N_B  =>  sparse == dense, dense == torch CPU SDPA (library routine).
  * D.4 diagnostics (orc_diag_cells / orc_roughness / orc_diag_summary): hand-worked examples D1-D3
  * (tests/golden/diag_examples.txt), closed forms (identical / alternating rows), numpy brute force.
+ * Per-row bitmap selection (orc_select_rows_bitmap, L269): numpy brute force, identical rows reduce to
+ * the per-tile selection, k_row >= N_B selects every visible block, count bounds.
  * Parity unpinned (conventions fixed by fiat): G5 (sigma := 1 when nothing is dropped),
  * G6 (tie-break: lower block index first), G7 (GQA mapping h -> h / (H/H_kv)), G9 (per-sequence
  * quantile; batch is looped by the caller).
@@ -436,6 +438,54 @@ void orc_diag_summary(const float* g, const float* r, const float* d2, const flo
     out[11] = (float)((double)gv[m40 - 1] / tau_hat);
   }
   free(gv); free(dv2);
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * Per-row selection scattered into a per-tile block bitmap (section 4.5 item 1: "A
+ * per-row scatter-into-bitmap kernel would close the rest of the gap without re-materialising the
+ * [B, H, M, N_B] keep tensor; not yet built").  SURVEY 8(f).4; reading G18:
+ *   every query row i of tile t ranks the visible blocks by ITS OWN row score s[i,h,b] (O3 / O3q; no
+ *   tile max), blocks 0 and t forced on top (Eq.9), ties -> lower block index (G6), and keeps its first
+ *   min(k_row, t+1) blocks; the tile's bitmap is the union over its Bn rows and the whole tile attends
+ *   the union (one bit per (tile, head, block) instead of one per (row, head, block)).
+ *   bitmap [n_tiles, H, NBW] uint32, NBW = ceil(N_B / 32), bit b%32 of word b/32;  count [n_tiles, H]
+ * ------------------------------------------------------------------------------------------- */
+void orc_select_rows_bitmap(const uint16_t* Q, const float* kmean, const uint16_t* kmin,
+                            const uint16_t* kmax, int64_t H, int64_t Hkv, int64_t N, int64_t d,
+                            int64_t Bn, int policy, int64_t k_row, const int64_t* tiles, int64_t n_tiles,
+                            uint32_t* bitmap, int32_t* count) {
+  int64_t NB = N / Bn, NBW = (NB + 31) / 32, G = H / Hkv;
+  int quest = (policy == POLICY_QUEST || policy == POLICY_ROUTER_QUEST);
+#pragma omp parallel
+  {
+    cand_t* scratch = (cand_t*)malloc(sizeof(cand_t) * (size_t)NB);
+#pragma omp for collapse(2) schedule(dynamic, 1)
+    for (int64_t it = 0; it < n_tiles; ++it)
+      for (int64_t h = 0; h < H; ++h) {
+        int64_t t = tiles[it], g = h / G;
+        uint32_t* bm = bitmap + (it * H + h) * NBW;
+        for (int64_t w = 0; w < NBW; ++w) bm[w] = 0;
+        int64_t f = (t == 0) ? 1 : 2, nf = t + 1 - f;
+        bm[0] |= 1u;                                       /* sink */
+        bm[t >> 5] |= 1u << (t & 31);                      /* self */
+        int64_t keep = k_row - f;
+        if (keep > nf) keep = nf;
+        for (int64_t r = 0; r < Bn && keep > 0; ++r) {
+          const uint16_t* q = Q + (h * N + t * Bn + r) * d;
+          for (int64_t i = 0; i < nf; ++i) {
+            int64_t b = i + 1, o = (g * NB + b) * d;
+            scratch[i].s = quest ? row_score_quest(q, kmin + o, kmax + o, d) : row_score_mean(q, kmean + o, d);
+            scratch[i].b = (int32_t)b;
+          }
+          qsort(scratch, (size_t)nf, sizeof(cand_t), cand_cmp);
+          for (int64_t i = 0; i < keep; ++i) bm[scratch[i].b >> 5] |= 1u << (scratch[i].b & 31);
+        }
+        int32_t c = 0;
+        for (int64_t w = 0; w < NBW; ++w) c += __builtin_popcount(bm[w]);
+        count[it * H + h] = c;
+      }
+    free(scratch);
+  }
 }
 
 int orc_max_threads(void) {

@@ -87,6 +87,12 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     lib.bsa_sparse_attn_fwd_varlen.restype = ctypes.c_int
     lib.bsa_dense_attn_fwd_varlen.argtypes = [sp, ip, i32, vp, vp, vp, ctypes.c_float, vp, vp, vp]
     lib.bsa_dense_attn_fwd_varlen.restype = ctypes.c_int
+    lib.bsa_bitmap_words.argtypes = [sp]
+    lib.bsa_bitmap_words.restype = sz
+    lib.bsa_select_rows_bitmap.argtypes = [sp, vp, vp, ctypes.c_int, i32, vp, vp, vp]
+    lib.bsa_select_rows_bitmap.restype = ctypes.c_int
+    lib.bsa_sparse_attn_fwd_bitmap.argtypes = [sp, vp, vp, vp, vp, ctypes.c_float, vp, vp, vp]
+    lib.bsa_sparse_attn_fwd_bitmap.restype = ctypes.c_int
     lib.bsa_last_error.restype = ctypes.c_char_p
     lib.bsa_version.restype = ctypes.c_char_p
     if path is None:
@@ -305,6 +311,34 @@ def bsa_dense_attn_fwd_varlen(Q, K, V, cu_seqlens, block: int, softmax_scale: fl
     lse = torch.empty(Q.shape[1] * Q.shape[2], dtype=torch.float32, device=Q.device) if want_lse else None
     _check(lib.bsa_dense_attn_fwd_varlen(ctypes.byref(shape), cu, n, _ptr(Q), _ptr(K), _ptr(V),
                                          float(softmax_scale), _ptr(O), _ptr(lse), _stream()))
+    return O, lse
+
+
+# ---- per-row selection scattered into a per-tile bitmap ----------------------------------
+def bsa_select_rows_bitmap(Q, meta, K_like, block: int, policy: str, k_row: int):
+    """Returns (bitmap int32-viewed uint32 [B,Hq,T,words], kv_count int32 [B,Hq,T])."""
+    lib = load_library()
+    shape = make_shape(Q, K_like, block)
+    B, H, N, _ = Q.shape
+    T = N // block
+    words = int(lib.bsa_bitmap_words(ctypes.byref(shape)))
+    bitmap = torch.empty((B, H, T, words), dtype=torch.int32, device=Q.device)
+    count = torch.empty((B, H, T), dtype=torch.int32, device=Q.device)
+    _check(lib.bsa_select_rows_bitmap(ctypes.byref(shape), _ptr(Q), _ptr(meta), POLICIES[policy], k_row,
+                                      _ptr(bitmap), _ptr(count), _stream()))
+    return bitmap, count
+
+
+def bsa_sparse_attn_fwd_bitmap(Q, K, V, bitmap, block: int, softmax_scale: float = 0.0,
+                               O: torch.Tensor | None = None, want_lse: bool = False):
+    lib = load_library()
+    shape = make_shape(Q, K, block)
+    if O is None:
+        O = torch.empty_like(Q)
+    lse = torch.empty(Q.shape[:3], dtype=torch.float32, device=Q.device) if want_lse else None
+    assert bitmap.dtype == torch.int32 and bitmap.is_contiguous()
+    _check(lib.bsa_sparse_attn_fwd_bitmap(ctypes.byref(shape), _ptr(Q), _ptr(K), _ptr(V), _ptr(bitmap),
+                                          float(softmax_scale), _ptr(O), _ptr(lse), _stream()))
     return O, lse
 
 

@@ -371,4 +371,47 @@ bsa_status bsa_dense_attn_fwd_varlen(const bsa_shape* shape, const int32_t* cu_s
                      stream);
 }
 
+/* ---- per-row selection scattered into a per-tile bitmap ---------------- */
+size_t bsa_bitmap_words(const bsa_shape* shape) {
+  Dims D;
+  if (make_dims(shape, &D) != BSA_OK) return 0;
+  return static_cast<size_t>((D.NB + 31) / 32);
+}
+
+bsa_status bsa_select_rows_bitmap(const bsa_shape* shape, const void* Q, const void* meta, bsa_policy policy,
+                                  int32_t k_row, uint32_t* bitmap, int32_t* kv_count, void* stream) {
+  Dims D;
+  bsa_status st = make_dims(shape, &D);
+  if (st != BSA_OK) return st;
+  if (!Q || !meta || !bitmap || !kv_count)
+    return fail(BSA_ERR_INVALID_ARG, "Q, meta, bitmap and kv_count must not be NULL");
+  if (policy != BSA_POLICY_TOPK && policy != BSA_POLICY_QUEST)
+    return fail(BSA_ERR_INVALID_ARG, "rows_bitmap: policy must be BSA_POLICY_TOPK (K-mean) or BSA_POLICY_QUEST");
+  if (k_row < 3) return fail(BSA_ERR_INVALID_ARG, "k_row %d < 3", k_row);
+  if (k_row > 64) return fail(BSA_ERR_UNSUPPORTED, "k_row %d > 64", k_row);
+  if (!aligned16(Q) || (reinterpret_cast<uintptr_t>(meta) & 255u))
+    return fail(BSA_ERR_INVALID_ARG, "Q must be 16-byte and meta 256-byte aligned");
+  st = check_device();
+  if (st != BSA_OK) return st;
+  return launch_rowsel(D, Q, meta, policy == BSA_POLICY_QUEST, k_row, bitmap, kv_count,
+                       static_cast<cudaStream_t>(stream));
+}
+
+bsa_status bsa_sparse_attn_fwd_bitmap(const bsa_shape* shape, const void* Q, const void* K, const void* V,
+                                      const uint32_t* bitmap, float softmax_scale, void* O, float* lse,
+                                      void* stream) {
+  Dims D;
+  bsa_status st = make_dims(shape, &D);
+  if (st != BSA_OK) return st;
+  if (!Q || !K || !V || !O || !bitmap) return fail(BSA_ERR_INVALID_ARG, "Q, K, V, O and bitmap must not be NULL");
+  if (!aligned16(Q) || !aligned16(K) || !aligned16(V) || !aligned16(O))
+    return fail(BSA_ERR_INVALID_ARG, "Q, K, V and O must be 16-byte aligned");
+  st = check_device();
+  if (st != BSA_OK) return st;
+  const float scale = softmax_scale > 0.f ? softmax_scale
+                                          : static_cast<float>(1.0 / sqrt(static_cast<double>(D.d)));
+  return launch_attn(D, Q, K, V, nullptr, nullptr, 0, true, scale, O, lse, static_cast<cudaStream_t>(stream),
+                     bitmap);
+}
+
 }  // extern "C"

@@ -56,8 +56,10 @@ struct Cfg {
 };
 
 struct Params {
-  const int32_t* kv_idx;    // [B,H,T,W] or nullptr (dense)
+  const int32_t* kv_idx;    // [B,H,T,W] or nullptr (dense, bitmap)
   const int32_t* kv_count;  // [B,H,T] or nullptr
+  const uint32_t* bitmap;   // [B,H,T,nbw] block bitmap per (tile, head) (rowsel.cu), or nullptr
+  int nbw;
   uint16_t* O;
   float* lse;
   int W, B, H, G, N, Bn, NB, NT;
@@ -73,7 +75,29 @@ struct alignas(8) Ctl {
   uint64_t kv_full[8], kv_empty[8];
   uint32_t tmem_base;
   int32_t n_valid;
-  uint16_t list[kMaxW];
+  union {
+    uint16_t list[kMaxW];       // kv_idx mode: the compacted row
+    uint32_t bmw[kMaxW / 2];    // bitmap mode: the row's words, masked to blocks <= t (N_B <= 4096)
+  };
+};
+
+// Walks the set bits of a bitmap row in ascending order; block_at(n) must be called with non-decreasing n.
+struct BitCursor {
+  const uint32_t* w;
+  int wi, idx, blk;
+  uint32_t cur;
+  __device__ __forceinline__ void init(const uint32_t* words) {
+    w = words; wi = 0; idx = -1; blk = -1; cur = words[0];
+  }
+  __device__ __forceinline__ int block_at(int n) {
+    while (idx < n) {
+      while (cur == 0u) cur = w[++wi];
+      blk = wi * 32 + __ffs(cur) - 1;
+      cur &= cur - 1u;
+      ++idx;
+    }
+    return blk;
+  }
 };
 static_assert(sizeof(Ctl) <= 1024, "Ctl must fit the 1 KB bookkeeping area");
 
@@ -406,7 +430,20 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
     __syncwarp();
     tmem_alloc<C::TMEM_COLS>(smem_u32(&ctl->tmem_base));
   }
-  if (SPARSE && warp == 0) {
+  if (SPARSE && warp == 0 && p.bitmap != nullptr) {
+    // bitmap mode: copy the row's words, masked to the visible blocks (<= t); count the set bits
+    const int64_t row = (static_cast<int64_t>(b) * p.H + h) * p.NT + tq;
+    const uint32_t* src = p.bitmap + row * p.nbw;
+    int cnt = 0;
+    for (int i = lane; i < kMaxW / 2; i += 32) {
+      uint32_t wv = (i < p.nbw && i * 32 <= tq) ? src[i] : 0u;
+      if (i == (tq >> 5) && (tq & 31) != 31) wv &= (2u << (tq & 31)) - 1u;
+      ctl->bmw[i] = wv;
+      cnt += __popc(wv);
+    }
+    cnt = __reduce_add_sync(0xffffffffu, cnt);
+    if (lane == 0) ctl->n_valid = cnt;
+  } else if (SPARSE && warp == 0) {
     // compact the valid entries of this kv_idx row (sentinel >= N_B and blocks > t are skipped, A.10;
     // a block listed more than once is attended once, like the oracle's O11)
     const int64_t row = (static_cast<int64_t>(b) * p.H + h) * p.NT + tq;
@@ -445,10 +482,20 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
     const int last = (q0 + BM < p.N ? q0 + BM : p.N);
     n_it = last / BN;
   }
-  auto key_start = [&](int j) -> int {
-    if (SPARSE) return ctl->list[j / SUBS] * p.Bn + (j % SUBS) * BN;
+  const bool use_bm = SPARSE && p.bitmap != nullptr;
+  BitCursor cur_a, cur_b;                      // softmax: cur_a; TMA producer: cur_a for K, cur_b for V
+  if (use_bm) {
+    cur_a.init(ctl->bmw);
+    cur_b.init(ctl->bmw);
+  }
+  auto start_of = [&](BitCursor& cur, int j) -> int {
+    if (SPARSE) {
+      const int blk = use_bm ? cur.block_at(j / SUBS) : static_cast<int>(ctl->list[j / SUBS]);
+      return blk * p.Bn + (j % SUBS) * BN;
+    }
     return j * BN;
   };
+  auto key_start = [&](int j) -> int { return start_of(cur_a, j); };
 
   // ---- K/V ring bookkeeping --------------------------------------------------------------------
   // BM = 128, d <= 128 (two CTAs per SM): one thread issues QK(j+1), PV(j) alternately (kAhead = 1)
@@ -476,17 +523,16 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
     if (warp == 4) {
       // ---- TMA producer: K(0..kAhead-1), then [K(j+kAhead), V(j)] for j = 0, 1, ... -------------
       if (lane == 0) {
-        auto load = [&](const CUtensorMap* tm, int j, int s, int seq, int ns) {
+        auto load = [&](const CUtensorMap* tm, int k0, int s, int seq, int ns) {
           mbar_wait(smem_u32(&ctl->kv_empty[s]), ((seq / ns) & 1) ^ 1);
           mbar_arrive_expect_tx(smem_u32(&ctl->kv_full[s]), C::KV_BYTES);
-          tma_load_5d(smem_u32(kv_s + s * C::KV_BYTES), tm, smem_u32(&ctl->kv_full[s]), 0,
-                      key_start(j), 0, g, b);
+          tma_load_5d(smem_u32(kv_s + s * C::KV_BYTES), tm, smem_u32(&ctl->kv_full[s]), 0, k0, 0, g, b);
         };
-        for (int i = 0; i < kAhead && i < n_it; ++i) load(&tmK, i, slot_k(i), seq_k(i), NSK);
+        for (int i = 0; i < kAhead && i < n_it; ++i) load(&tmK, start_of(cur_a, i), slot_k(i), seq_k(i), NSK);
         for (int j = 0; j < n_it; ++j) {
           const int i = j + kAhead;
-          if (i < n_it) load(&tmK, i, slot_k(i), seq_k(i), NSK);
-          load(&tmV, j, slot_v(j), seq_v(j), NSV);
+          if (i < n_it) load(&tmK, start_of(cur_a, i), slot_k(i), seq_k(i), NSK);
+          load(&tmV, start_of(cur_b, j), slot_v(j), seq_v(j), NSV);
         }
       }
     } else if (warp == 5 || warp == 6) {
@@ -597,10 +643,15 @@ bsa_status run(const Dims& S, const void* Q, const void* K, const void* V, const
 
 bsa_status launch_attn(const Dims& S, const void* Q, const void* K, const void* V,
                        const int32_t* kv_idx, const int32_t* kv_count, int W, bool sparse, float scale,
-                       void* O, float* lse, cudaStream_t stream) {
+                       void* O, float* lse, cudaStream_t stream, const uint32_t* bitmap) {
   Params prm;
   prm.kv_idx = kv_idx;
   prm.kv_count = kv_count;
+  prm.bitmap = bitmap;
+  prm.nbw = (S.NB + 31) / 32;
+  if (bitmap && S.NB > 32 * (kMaxW / 2))
+    return fail(BSA_ERR_UNSUPPORTED, "bitmap attention: %d blocks per sequence, at most %d", S.NB,
+                32 * (kMaxW / 2));
   prm.O = static_cast<uint16_t*>(O);
   prm.lse = lse;
   prm.W = W;
@@ -608,7 +659,7 @@ bsa_status launch_attn(const Dims& S, const void* Q, const void* K, const void* 
   prm.qsb = S.qsb; prm.qsh = S.qsh; prm.qsn = S.qsn;
   prm.scale_log2 = scale * 1.4426950408889634f;
   if (sparse) {
-    if (W > kMaxW) return fail(BSA_ERR_UNSUPPORTED, "sparse attn: kv_width %d > %d", W, kMaxW);
+    if (!bitmap && W > kMaxW) return fail(BSA_ERR_UNSUPPORTED, "sparse attn: kv_width %d > %d", W, kMaxW);
     prm.NT = S.NB;
 #define BSA_SP(BMM, DD) \
   if (S.Bn == BMM && S.d == DD) return run<BMM, DD, true>(S, Q, K, V, prm, stream);

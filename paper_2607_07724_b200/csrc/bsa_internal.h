@@ -54,8 +54,12 @@ bsa_status launch_score_tc_mean(const Dims& D, const void* Q, const void* meta, 
 // per-sequence reduction of the D.4 per-cell quantities (diag.cu)
 bsa_status launch_diag_summary(const Dims& D, int k, int router, const float* tau, const SelectDiag& dg,
                                cudaStream_t stream);
+// per-row selection scattered into a per-tile bitmap (rowsel.cu)
+bsa_status launch_rowsel(const Dims& D, const void* Q, const void* meta, bool quest, int k_row,
+                         uint32_t* bitmap, int32_t* count, cudaStream_t stream);
 bsa_status launch_attn(const Dims& D, const void* Q, const void* K, const void* V,
                        const int32_t* kv_idx, const int32_t* kv_count, int W, bool sparse,
-                       float scale, void* O, float* lse, cudaStream_t stream);
+                       float scale, void* O, float* lse, cudaStream_t stream,
+                       const uint32_t* bitmap = nullptr);
 
 }  // namespace bsa

@@ -677,7 +677,7 @@ def test_sparse_attention_duplicate_entries(bsa):
     orc = oracle.select(inp.Q, meta_np, cfg.block, "router", cfg.k_budget, 1.0)     # W = 8, all triggered
     idx = orc["kv_idx"].copy()
     W = idx.shape[-1]
-    wide = np.full((H, T, 40), NB, np.int32)                 # two chunks of 32 -> cross-chunk duplicates
+    wide = np.full((H, T, 48), NB, np.int32)                 # two chunks of 32 -> cross-chunk duplicates
     wide[:, :, :W] = idx
     wide[:, :, W:2 * W] = idx                                # every entry twice, same chunk
     wide[:, :, 33:33 + W] = idx                              # and a third time in the second chunk
@@ -810,3 +810,75 @@ def test_varlen_three_lengths(bsa, policy):
         Odg = Od[0, :, s0:s0 + cfg.seqlen].float().cpu().numpy().reshape(H, T, block, cfg.head_dim)
         compare_attn(np.stack([Odg[h, t] for t, h in pairs]), refd, f"varlen[{i}] dense")
     assert len(set(taus)) == len(taus), "the quantile threshold is per sequence (G9)"
+
+
+# ---- per-row selection scattered into a per-tile bitmap -------------------
+def _row_scores_np(inp, meta_np, cfg, policy, t, h):
+    """fp32 row scores [Bn, t+1] of one (tile, head), independent numpy formulation (for tie checks)."""
+    import math
+    kmean, kmin, kmax = meta_np
+    g = h // cfg.group
+    q = bf16_to_f32(inp.Q[h, t * cfg.block:(t + 1) * cfg.block]).astype(np.float64)
+    if policy == "quest":
+        s = np.maximum(q, 0) @ bf16_to_f32(kmax[g, :t + 1]).astype(np.float64).T + \
+            np.minimum(q, 0) @ bf16_to_f32(kmin[g, :t + 1]).astype(np.float64).T
+        return s.astype(np.float32)
+    return (q @ kmean[g, :t + 1].astype(np.float64).T).astype(np.float32) * np.float32(1 / math.sqrt(cfg.head_dim))
+
+
+ROWSEL_CASES = [("C1", "topk", 3), ("C1", "quest", 4), ("C1odd", "topk", 5), ("C2s", "quest", 8),
+                ("C2s", "topk", 4), ("C5s", "quest", 6), ("C5s", "topk", 4), ("C2m", "quest", 6),
+                ("C2m", "topk", 33)]
+
+
+@pytest.mark.parametrize("name,policy,k_row", ROWSEL_CASES)
+def test_rows_bitmap_parity(bsa, name, policy, k_row):
+    """bsa_select_rows_bitmap vs oracle.select_rows_bitmap (bit-exact outside near-ties of a row's cutoff),
+    then bsa_sparse_attn_fwd_bitmap fed the ORACLE's bitmap vs oracle attention over the same blocks."""
+    import torch
+    from parity_util import TIE_REL
+    if name == "C2m" and name not in _CACHE:
+        cfg = synth.CONFIGS["C2"].scaled(16384, name)
+        inp = synth.make_inputs(cfg)
+        _CACHE[name] = (cfg, inp, oracle.pool(inp.K, cfg.block))
+    cfg, inp, meta_np = _case(name)
+    Q, K, V = _dev(inp)
+    T, H, NB = cfg.n_blocks, cfg.n_q_heads, cfg.n_blocks
+    buf = _meta_from_oracle(bsa, meta_np, K, cfg.block)
+    bm, cnt = bsa.bsa_select_rows_bitmap(Q, buf, K, cfg.block, policy, k_row)
+    torch.cuda.synchronize()
+    o_bm, o_cnt = oracle.select_rows_bitmap(inp.Q, meta_np, cfg.block, policy, k_row)    # [T, H, words]
+    g_bm = bm[0].cpu().numpy().view(np.uint32).transpose(1, 0, 2)                         # -> [T, H, words]
+    g_cnt = cnt[0].cpu().numpy().T
+    gb = np.unpackbits(np.ascontiguousarray(g_bm).view(np.uint8), axis=-1, bitorder="little")[..., :NB]
+    ob = np.unpackbits(o_bm.view(np.uint8), axis=-1, bitorder="little")[..., :NB]
+    assert np.array_equal(g_cnt, gb.sum(-1)), "kv_count is the popcount of the row"
+    tt = np.arange(T)
+    assert gb[:, :, 0].all() and gb[tt, :, tt].all(), "forced sink / self"
+    diff_cells = np.argwhere((gb != ob).any(-1))
+    records = []
+    for t, h in diff_cells:
+        s = _row_scores_np(inp, meta_np, cfg, policy, t, h)                # [Bn, t+1]
+        keep = min(k_row - 2, t - 1)
+        kth = -np.sort(-s[:, 1:t], axis=1)[:, keep - 1:keep + 1]          # scores at the row cut-offs
+        for b in np.nonzero(gb[t, h] != ob[t, h])[0]:
+            near = np.abs(s[:, b:b + 1] - kth) <= TIE_REL * np.maximum(np.abs(s[:, b:b + 1]), np.abs(kth))
+            assert near.any(), f"{name}/{policy} t={t} h={h}: block {b} differs outside every row's tie band"
+        records.append(dict(kind="bitmap", t=int(t), h=int(h),
+                            blocks=np.nonzero(gb[t, h] != ob[t, h])[0].tolist()))
+    assert len(diff_cells) <= max(2, T * H // 50)
+    _log(f"{name}/{policy}/k_row={k_row}", dict(stage="rows_bitmap", cells=T * H, tie_cells=len(diff_cells),
+                                                 mean_blocks=float(ob.sum(-1).mean())), records)
+    # attention from the ORACLE's bitmap
+    if NB <= 4096:
+        obm_dev = torch.from_numpy(np.ascontiguousarray(o_bm.transpose(1, 0, 2)).view(np.int32))[None].cuda()
+        O, lse = bsa.bsa_sparse_attn_fwd_bitmap(Q, K, V, obm_dev, cfg.block, want_lse=True)
+        torch.cuda.synchronize()
+        kv_idx, kv_count = oracle.bitmap_to_kv_idx(o_bm, NB)
+        ts = sorted(set([0, 1, 2, min(T - 1, k_row), T // 2, T - 1]))
+        pairs = [(t, h) for h in sorted({0, H - 1}) for t in ts]
+        ref, ref_lse = oracle.attn_pairs(inp.Q, inp.K, inp.V, cfg.block, pairs, kv_idx, kv_count)
+        Og = O[0].float().cpu().numpy().reshape(H, T, cfg.block, cfg.head_dim)
+        Lg = lse[0].cpu().numpy().reshape(H, T, cfg.block)
+        compare_attn(np.stack([Og[h, t] for t, h in pairs]), ref, f"bitmap attention {name}/{policy}")
+        np.testing.assert_allclose(np.stack([Lg[h, t] for t, h in pairs]), ref_lse, rtol=0, atol=2e-3)
