@@ -18,7 +18,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libbsa.so")
 STAMP = LIB + ".srchash"
-SOURCES = ["api.cu", "pool.cu", "select.cu", "score_tc_quest.cu", "score_tc_mean.cu", "attn.cu", "diag.cu", "rowsel.cu"]
+SOURCES = ["api.cu", "pool.cu", "select.cu", "score_tc_quest.cu", "score_tc_mean.cu", "attn.cu", "attn_t.cu", "diag.cu", "rowsel.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 NVCC_FLAGS += shlex.split(os.environ.get("BSA_NVCC_FLAGS", ""))   # developer knob, e.g. -DBSA_TC_OCC2=0

@@ -14,6 +14,7 @@
 // Q tile rows: sparse = one selection tile (BM = block), dense = 128.  For BM = 64 the accumulator
 // rows live in lanes 0-15 of each TMEM sub-partition (UMMA M = 64 layout).
 #include <cuda_bf16.h>
+#include <stdlib.h>
 
 #include "bsa_internal.h"
 #include "sm100_ptx.cuh"
@@ -641,6 +642,14 @@ bsa_status run(const Dims& S, const void* Q, const void* K, const void* V, const
 
 }  // namespace
 
+// The transposed kernel of attn_t.cu (keys on the M dimension, M = 128) is parity-green but slower than
+// the M = 64 kernel here on B200 (C2: 2.3-2.7 ms against 1.5 ms; ablation in DESIGN.md section 6), so it
+// is an opt-in experiment: the environment variable BSA_ATTN_T=1 routes block 64 / head_dim 128 to it.
+static bool attn_t_enabled() {
+  const char* e = getenv("BSA_ATTN_T");
+  return e != nullptr && e[0] == '1';
+}
+
 bsa_status launch_attn(const Dims& S, const void* Q, const void* K, const void* V,
                        const int32_t* kv_idx, const int32_t* kv_count, int W, bool sparse, float scale,
                        void* O, float* lse, cudaStream_t stream, const uint32_t* bitmap) {
@@ -658,6 +667,8 @@ bsa_status launch_attn(const Dims& S, const void* Q, const void* K, const void* 
   prm.B = S.B; prm.H = S.H; prm.G = S.G; prm.N = S.N; prm.Bn = S.Bn; prm.NB = S.NB;
   prm.qsb = S.qsb; prm.qsh = S.qsh; prm.qsn = S.qsn;
   prm.scale_log2 = scale * 1.4426950408889634f;
+  if (sparse && !bitmap && attn_t_supported(S, W) && attn_t_enabled())
+    return launch_attn_t(S, Q, K, V, kv_idx, kv_count, W, scale, O, lse, stream);
   if (sparse) {
     if (!bitmap && W > kMaxW) return fail(BSA_ERR_UNSUPPORTED, "sparse attn: kv_width %d > %d", W, kMaxW);
     prm.NT = S.NB;

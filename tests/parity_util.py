@@ -18,7 +18,7 @@ SIGMA_BAR_BAND = 1e-5   # a trigger may differ only on tiles with |sigma_bar - t
                         # protocol item 1); each such tile is logged with its gap, never hidden
 ATTN_MAX_ABS = 2e-2
 ATTN_MEAN_ABS = 2e-3
-
+LSE_TOL = 2e-3          # log-sum-exp of the scaled logits (fp32 row sums of the unrounded p)
 
 def to_torch_bf16(bits: np.ndarray, device="cuda"):
     import torch
