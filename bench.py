@@ -552,7 +552,7 @@ def run_gpu(args):
         from dataclasses import replace
         del run
         torch.cuda.empty_cache()
-        extra, sweeps = {}, {}
+        extra, sweeps, line_next = {}, {}, {}
         n_x, w_x = max(3, min(args.steps, 8)), 2
         plans = [("C2", ("router_quest", "topk", "quest", "router")), ("C3a", ("router_quest", "topk")),
                  ("C3b", ("topk",)), ("C4", ("router_quest", "quest")), ("C5", ("router_quest", "router")),
@@ -591,8 +591,46 @@ def run_gpu(args):
                     sweeps[f"k={kb}/{pol}/q={qf}"] = rec
                     del r2
                     torch.cuda.empty_cache()
+            if name == "C2":   # SURVEY 8(f).3 / 8(f).4 on the 32K layer: diagnostics mode, per-row bitmap
+                r2 = Runner(c, i2, "router_quest", args.q_frac, torch, bsa)
+                next_rows = {}
+
+                def timed(fn, n=5):
+                    ts = []
+                    for i in range(n + 2):
+                        r2.flush_l2()
+                        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                        e0.record()
+                        fn()
+                        e1.record()
+                        torch.cuda.synchronize()
+                        if i >= 2:
+                            ts.append(e0.elapsed_time(e1))
+                    return float(np.median(ts))
+
+                bsa.bsa_build_block_meta(r2.K, c.block, 3, r2.meta)
+                next_rows["select_ms"] = timed(lambda: bsa.bsa_select(
+                    r2.Q, r2.meta, r2.K, c.block, "router_quest", c.k_budget, args.q_frac, out=r2.sel))
+                dsel = dict(r2.sel)
+                next_rows["select_diag_ms"] = timed(lambda: dsel.update(bsa.bsa_select(
+                    r2.Q, r2.meta, r2.K, c.block, "router_quest", c.k_budget, args.q_frac, out=dsel, diag=True)))
+                next_rows["diag_summary"] = dict(zip(bsa.DIAG_SUMMARY, dsel["summary"][0].cpu().tolist()))
+                for k_row in (4, 8):
+                    box = {}
+                    ms = timed(lambda: box.update(zip(("bm", "cnt"), bsa.bsa_select_rows_bitmap(
+                        r2.Q, r2.meta, r2.K, c.block, "quest", k_row))))
+                    cnt = int(box["cnt"].sum().item())
+                    ms_a = timed(lambda: bsa.bsa_sparse_attn_fwd_bitmap(r2.Q, r2.K, r2.V, box["bm"], c.block, O=r2.O))
+                    a2 = algorithmic(c, cnt)
+                    next_rows[f"rows_bitmap/quest/k_row={k_row}"] = {
+                        "select_rows_bitmap_ms": ms, "bitmap_attn_ms": ms_a,
+                        "mean_blocks_per_tile": cnt / (c.n_q_heads * c.n_blocks),
+                        "bitmap_attn_tflops": a2["sparse_flops"] / (ms_a * 1e-3) / 1e12}
+                line_next = next_rows
+                del r2, dsel
+                torch.cuda.empty_cache()
             del i2
-        line["extra"] = {"configs": extra, "sweeps": sweeps,
+        line["extra"] = {"configs": extra, "sweeps": sweeps, "next_rows_c2": line_next,
                          "note": f"{n_x} timed steps after {w_x} warm-ups per entry (C3c: 2), dense kernel timed "
                                  "once per config; sweeps at C2 (32K), 3 steps"}
 

@@ -72,6 +72,7 @@ struct PoolArgs {
   const uint16_t* K;
   int64_t ksb, ksh, ksn;
   int NB, Hkv, B, kinds;
+  int dfull;   // head_dim; a CTA covers D of its columns, starting at blockIdx.y * D
   float* kmean;
   uint16_t *kmin, *kmax, *ksplit;
   size_t plane_elems;
@@ -83,7 +84,8 @@ __device__ __forceinline__ void load_block(const PoolArgs<D, BN>& a, int w, uint
   constexpr int kThreads = BN * D / 64, TPR = D / 8, RPP = kThreads / TPR;
   const int blk = w % a.NB, g = (w / a.NB) % a.Hkv, b = w / (a.NB * a.Hkv);
   const int c8 = threadIdx.x % TPR, r0 = threadIdx.x / TPR;
-  const uint16_t* base = a.K + b * a.ksb + g * a.ksh + static_cast<int64_t>(blk) * BN * a.ksn + c8 * 8;
+  const uint16_t* base = a.K + b * a.ksb + g * a.ksh + static_cast<int64_t>(blk) * BN * a.ksn + c8 * 8 +
+                         blockIdx.y * D;
 #pragma unroll
   for (int p = 0; p < kPasses; ++p)
     v[p] = ld_stream(reinterpret_cast<const uint4*>(base + static_cast<int64_t>(r0 + p * RPP) * a.ksn));
@@ -192,7 +194,7 @@ __device__ __forceinline__ void process_block(const PoolArgs<D, BN>& a, int w, c
       lo = fminf(lo, (c & 1) ? bf_hi(wn) : bf_lo(wn));
       hv = fmaxf(hv, (c & 1) ? bf_hi(wx) : bf_lo(wx));
     }
-    const size_t o = ((static_cast<size_t>(b) * Hkv + g) * NB + blk) * D + c;
+    const size_t o = ((static_cast<size_t>(b) * Hkv + g) * NB + blk) * a.dfull + blockIdx.y * D + c;
     if (kinds & BSA_META_MEAN) {
       const float mean = static_cast<float>(s / static_cast<double>(BN));  // Eq.1, rounded once
       kmean[o] = mean;
@@ -226,6 +228,7 @@ void launch(const Dims& S, const void* K, int kinds, char* meta, const MetaLayou
   a.K = static_cast<const uint16_t*>(K);
   a.ksb = S.ksb; a.ksh = S.ksh; a.ksn = S.ksn;
   a.NB = S.NB; a.Hkv = S.Hkv; a.B = S.B; a.kinds = kinds;
+  a.dfull = S.d;
   a.kmean = reinterpret_cast<float*>(meta + L.off_mean);
   a.kmin = reinterpret_cast<uint16_t*>(meta + L.off_min);
   a.kmax = reinterpret_cast<uint16_t*>(meta + L.off_max);
@@ -235,7 +238,9 @@ void launch(const Dims& S, const void* K, int kinds, char* meta, const MetaLayou
   const int total = S.NB * S.Hkv * S.B;
   // one block per CTA: with ~6 CTAs resident per SM their load and reduce phases interleave; a
   // persistent register-double-buffered variant measured 25 % slower (fewer warps to hide the adds)
-  pool_kernel<D, BN><<<total, kThreads, 0, stream>>>(a);
+  // head_dim 256 runs as two 128-column halves (blockIdx.y): 512-thread CTAs at 128 registers left one
+  // CTA of 16 warps per SM (ncu r02: 22.8 % occupancy, 3.1 TB/s); the halves are the d = 128 kernel
+  pool_kernel<D, BN><<<dim3(total, S.d / D), kThreads, 0, stream>>>(a);
 }
 
 }  // namespace
@@ -247,10 +252,10 @@ bsa_status launch_pool(const Dims& S, const void* K, int kinds, void* meta, cuda
   if (S.d == DD && S.Bn == BB) { launch<DD, BB>(S, K, kinds, m, L, stream); return check_launch("pool_kernel"); }
   BSA_POOL_CASE(64, 64)
   BSA_POOL_CASE(128, 64)
-  BSA_POOL_CASE(256, 64)
+  if (S.d == 256 && S.Bn == 64) { launch<128, 64>(S, K, kinds, m, L, stream); return check_launch("pool_kernel"); }
   BSA_POOL_CASE(64, 128)
   BSA_POOL_CASE(128, 128)
-  BSA_POOL_CASE(256, 128)
+  if (S.d == 256 && S.Bn == 128) { launch<128, 128>(S, K, kinds, m, L, stream); return check_launch("pool_kernel"); }
 #undef BSA_POOL_CASE
   return fail(BSA_ERR_UNSUPPORTED, "pool: unsupported head_dim %d / block %d", S.d, S.Bn);
 }

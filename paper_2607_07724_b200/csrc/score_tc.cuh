@@ -76,7 +76,7 @@ struct TcParams {
   int32_t* kv_idx;
   int32_t* kv_count;
   float* sigma;
-  int B, H, Hkv, G, NB, k, W, router, sets, stages, nbpad, n_items;
+  int B, H, Hkv, G, NB, k, W, router, sets, stages, nbpad, n_items, ncand;
   float inv_sqrt_d;
   // D.4 diagnostics (Eq.18), all [B,H,T] or nullptr (diag == 0)
   int diag;
@@ -114,7 +114,7 @@ __device__ __forceinline__ Item decode_item(const TcParams& p, int w) {
   return it;
 }
 
-template <int D, int BN, bool QUEST, int NH>
+template <int D, int BN, bool QUEST, int NH, bool DIAG>
 __global__ void __launch_bounds__(kTcThreads, 1)
 score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmA,
                 const TcParams p) {
@@ -124,8 +124,10 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   uint8_t* a_s = smem + C::B_BYTES;                      // ring of [128 x 128 B] stages
   uint32_t* sc = reinterpret_cast<uint32_t*>(a_s + p.stages * kAStageBytes);   // [NH][nbpad] okey(score)
   unsigned long long* cand = reinterpret_cast<unsigned long long*>(sc + C::NH * p.nbpad);
-  uint32_t* srt = reinterpret_cast<uint32_t*>(cand + C::NH * kMaxCand);   // sorted keys (diag), per head
-  TcCtl* ctl = reinterpret_cast<TcCtl*>(srt + C::NH * kMaxCand);
+  // candidate / sorted-key arrays are sized by the budget (p.ncand >= 2k + 1 entries per head), the sorted
+  // keys exist only in diagnostics mode: at N_B = 4096 these bytes decide whether four heads fit
+  uint32_t* srt = reinterpret_cast<uint32_t*>(cand + C::NH * p.ncand);    // sorted keys (diag), per head
+  TcCtl* ctl = reinterpret_cast<TcCtl*>(srt + (DIAG ? C::NH * p.ncand : 0));
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int w0 = static_cast<int>(blockIdx.x), wstep = static_cast<int>(gridDim.x);
@@ -282,9 +284,9 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         tc_fence_after();
         const int blk = c * kABlocks + warp * 32 + lane;
         const uint32_t tD = tmem + lane_base + buf * C::NROWS;
-#pragma unroll
-        for (int j = 0; j < C::NH; ++j) {
-          if (j >= im.nh) break;
+#pragma unroll(DIAG ? C::NH : 1)
+        for (int j = 0; j < (DIAG ? C::NH : im.nh); ++j) {
+          if (DIAG && j >= im.nh) break;
           float m0 = -INFINITY, m1 = -INFINITY, m2 = -INFINITY, m3 = -INFINITY;   // four independent chains
           float rs = 0.0f, prev = 0.0f;   // diag: sum of squared differences of adjacent rows' scores
 #pragma unroll
@@ -300,7 +302,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
               m2 = fmax3(m2, __uint_as_float(ra[i + 2]), __uint_as_float(rb[i + 2]));
               m3 = fmax3(m3, __uint_as_float(ra[i + 3]), __uint_as_float(rb[i + 3]));
             }
-            if (p.diag) {   // warp-uniform; rows c0 .. c0+63 are ra[0..31], rb[0..31]
+            if constexpr (DIAG) {   // rows c0 .. c0+63 are ra[0..31], rb[0..31]
               if (c0 > 0) { const float d0 = __uint_as_float(ra[0]) - prev; rs = fmaf(d0, d0, rs); }
 #pragma unroll
               for (int i = 0; i < 31; ++i) {
@@ -316,13 +318,13 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           }
           const float mx = fmaxf(fmax3(m0, m1, m2), m3);
           if (blk <= im.t) sc[j * p.nbpad + blk] = okey(QUEST ? mx : mx * p.inv_sqrt_d);   // Eq.3 (G8)
-          if (p.diag) rough[j] += (blk <= im.t) ? static_cast<double>(rs) : 0.0;
+          if constexpr (DIAG) rough[j] += (blk <= im.t) ? static_cast<double>(rs) : 0.0;
         }
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(smem_u32(&ctl->acc_empty[buf]));
       }
-      if (p.diag) {   // fixed-order reduction: lanes by shuffle tree, warps summed 0..3 by the consumer
+      if constexpr (DIAG) {   // fixed-order reduction: lanes by shuffle tree, warps summed 0..3 by the consumer
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
           double v = rough[j];
@@ -346,16 +348,16 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         const int h = im.h0 + sw;
         const int64_t row = (static_cast<int64_t>(im.b) * p.H + h) * p.NB + im.t;
         float rough_sum = 0.0f;
-        if (p.diag)   // read before the keys are released: the epilogue warps rewrite it for the next item
+        if constexpr (DIAG)   // read before the keys are released: the epilogue warps rewrite it for the next item
           rough_sum = ((ctl->rough[0][sw] + ctl->rough[1][sw]) + ctl->rough[2][sw]) + ctl->rough[3][sw];
         DiagCell cell;
         const float sig = warp_select(sc + sw * p.nbpad, im.t, p.k, p.NB, p.W, p.kv_idx + row * p.W,
-                                      cand + sw * kMaxCand, ctl->s3 + sw * 4, lane, rel,
-                                      p.diag ? &cell : nullptr, srt + sw * kMaxCand);
+                                      cand + sw * p.ncand, ctl->s3 + sw * 4, lane, rel,
+                                      DIAG ? &cell : nullptr, srt + sw * p.ncand);
         if (lane == 0) {
           p.sigma[row] = sig;
           if (!p.router) p.kv_count[row] = (p.k < im.t + 1) ? p.k : im.t + 1;
-          if (p.diag) {
+          if constexpr (DIAG) {
             p.dg_g[row] = cell.g;
             p.dg_G[row] = cell.G;
             p.dg_r[row] = cell.r;
@@ -380,11 +382,14 @@ struct DiagPtrs {
   float *g, *G, *r, *d2, *rough;   // all nullptr: no diagnostics
 };
 
+inline int tc_ncand(int k) { return (2 * k + 1 + 7) & ~7; }   // <= kMaxCand for k <= 128
+
 template <int D, int BN, bool QUEST, int NH>
-size_t tc_fixed_smem(int nbpad) {
+size_t tc_fixed_smem(int nbpad, int k, bool diag) {
   using C = TcCfg<D, BN, QUEST, NH>;
+  const size_t ncand = static_cast<size_t>(tc_ncand(k));
   return static_cast<size_t>(C::B_BYTES) + static_cast<size_t>(NH) * nbpad * 4 +
-         static_cast<size_t>(NH) * kMaxCand * 8 + static_cast<size_t>(NH) * kMaxCand * 4 + sizeof(TcCtl);
+         static_cast<size_t>(NH) * ncand * 8 + (diag ? static_cast<size_t>(NH) * ncand * 4 : 0) + sizeof(TcCtl);
 }
 constexpr size_t kTcSmemBudget = 227 * 1024;
 
@@ -404,7 +409,8 @@ bsa_status run_score_tc(const Dims& S, const void* Q, const char* meta, const Me
   const long long n_items = static_cast<long long>(S.NB) * S.B * S.Hkv * p.sets;
   if (n_items > 0x7fffffffLL) return fail(BSA_ERR_UNSUPPORTED, "select: too many work items");
   p.n_items = static_cast<int>(n_items);
-  const size_t fixed = tc_fixed_smem<D, BN, QUEST, NH>(p.nbpad);
+  p.ncand = tc_ncand(k);
+  const size_t fixed = tc_fixed_smem<D, BN, QUEST, NH>(p.nbpad, k, p.diag != 0);
   int stages = static_cast<int>((kTcSmemBudget - fixed) / kAStageBytes);
   p.stages = stages > kMaxStages ? kMaxStages : stages;
 #ifdef BSA_TC_STAGE_CAP
@@ -426,7 +432,7 @@ bsa_status run_score_tc(const Dims& S, const void* Q, const char* meta, const Me
     if (!make_tmap_bf16(&ta, base, 5, dims, strides, box))
       return fail(BSA_ERR_CUDA, "select: cuTensorMapEncodeTiled(meta) failed");
   }
-  auto kern = score_tc_kernel<D, BN, QUEST, NH>;
+  auto kern = p.diag ? score_tc_kernel<D, BN, QUEST, NH, true> : score_tc_kernel<D, BN, QUEST, NH, false>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        static_cast<int>(smem));
   if (e != cudaSuccess) return fail(BSA_ERR_CUDA, "select: smem attribute: %s", cudaGetErrorString(e));
@@ -444,7 +450,8 @@ bsa_status dispatch_nh(const Dims& S, const void* Q, const char* meta, const Met
   const int nbpad = (S.NB + 3) & ~3;
   // fewer heads per item than the GQA group has only cost A-plane re-reads; more never help
   const bool useful = (NH == 1) || (NH - 1 < S.G);
-  if (useful && tc_fixed_smem<D, BN, QUEST, NH>(nbpad) + 2 * kAStageBytes <= kTcSmemBudget)
+  const bool diag = dg.g != nullptr;
+  if (useful && tc_fixed_smem<D, BN, QUEST, NH>(nbpad, k, diag) + 2 * kAStageBytes <= kTcSmemBudget)
     return run_score_tc<D, BN, QUEST, NH>(S, Q, meta, L, k, W, router, kv_idx, kv_count, sigma, dg, stream);
   if constexpr (NH > 1) {
     return dispatch_nh<D, BN, QUEST, NH - 1>(S, Q, meta, L, k, W, router, kv_idx, kv_count, sigma, dg, stream);
@@ -452,8 +459,8 @@ bsa_status dispatch_nh(const Dims& S, const void* Q, const char* meta, const Met
     return fail(BSA_ERR_UNSUPPORTED,
                 "select: %d blocks per sequence need %zu bytes of shared memory per head (limit %zu): "
                 "at most %zu blocks fit for head_dim %d / block %d / this backbone",
-                S.NB, tc_fixed_smem<D, BN, QUEST, 1>(nbpad) + 2 * kAStageBytes, kTcSmemBudget,
-                (kTcSmemBudget - tc_fixed_smem<D, BN, QUEST, 1>(0) - 2 * kAStageBytes) / 4, S.d, S.Bn);
+                S.NB, tc_fixed_smem<D, BN, QUEST, 1>(nbpad, k, diag) + 2 * kAStageBytes, kTcSmemBudget,
+                (kTcSmemBudget - tc_fixed_smem<D, BN, QUEST, 1>(0, k, diag) - 2 * kAStageBytes) / 4, S.d, S.Bn);
   }
 }
 
