@@ -455,7 +455,9 @@ attn_t_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
             for (int ks = 0; ks < 4; ++ks) {
               const uint64_t ad = umma_smem_desc(k_a + ks * 32, 16, 1024);
               const uint64_t bd = umma_smem_desc(q_a + s * (TB * 128) + ks * 32, 16, 1024);
+#ifndef T_ABL_NOMMA
               umma_ss(tS, ad, bd, idesc, (s > 0) || (ks > 0));
+#endif
             }
             tc_commit(smem_u32(&ctl->k_empty[slot]));
           }
@@ -482,7 +484,9 @@ attn_t_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
             for (int ks = 0; ks < 4; ++ks) {
               const uint64_t ad = umma_smem_desc(v_a + ks * 2048, TB * 128, 1024);        // d chunks 8 KB apart
               const uint64_t bd = umma_smem_desc(p_a + (u * 4 + ks) * 2048, 16, 1024);
+#if !defined(T_ABL_NOMMA) && !defined(T_ABL_NOPV)
               umma_ss(tO, ad, bd, idesc, (jj > 0) || (u > 0) || (ks > 0));
+#endif
             }
             tc_commit(smem_u32(&ctl->v_empty[slot]));
             ++vseq;

@@ -61,106 +61,154 @@ struct alignas(8) RsCtl {
 
 __device__ __forceinline__ void bar128() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
 
-// One warp merges a segment into one row's running list.  keys[i], i in [j_lo, j_hi), are the keys of
-// blocks blk0 + i of this segment (candidates: free blocks only); list[0..np) = the row's current top
-// entries (key, block), blocks ascending, all below blk0.  Afterwards list holds the top
-// min(kprime, np + n_seg) of the union by (key desc, block asc), blocks ascending.  Returns the new np.
+// One warp merges a segment into the running lists of FOUR rows.  Per row: keys[i], i in [j_lo, j_hi), are
+// the keys of blocks blk0 + i of this segment (candidates: free blocks only); list[0..np) = the row's current
+// top entries (key, block), blocks ascending, all below blk0.  Afterwards list holds the top
+// min(kprime, np + n_seg) of the union by (key desc, block asc), blocks ascending, and np4[] the new counts.
+// The threshold is found by bisection on the key bits (ties to the lower block, warp_topk_compact's rule);
+// the four rows' (compare, redux) chains are independent and overlap their latencies.
 template <int KPL>
-__device__ __noinline__ int row_merge(const uint32_t* keys, int j_lo, int j_hi, int blk0, uint2* list,
-                                         int np, int kprime, int lane) {
+__device__ __noinline__ void row_merge4(const uint32_t* keys0, int seg, int j_lo, int j_hi, int blk0,
+                                        uint2* list0, int kcap, int16_t* np4, int kprime, int lane) {
   const unsigned full = 0xffffffffu;
-  uint32_t r[KPL], ck[2], cb[2];
-  uint32_t hi = 0u, lo = 0xffffffffu;
-#pragma unroll
-  for (int j = 0; j < KPL; ++j) {
-    const int i = j * 32 + lane;
-    const bool v = i >= j_lo && i < j_hi;
-    r[j] = v ? keys[i] : 0u;            // 0 is below the key of every score
-    hi = max(hi, r[j]);
-    lo = v ? min(lo, r[j]) : lo;
-  }
-#pragma unroll
-  for (int j = 0; j < 2; ++j) {
-    const int i = j * 32 + lane;
-    const bool v = i < np;
-    const uint2 e = v ? list[i] : make_uint2(0u, 0u);
-    ck[j] = e.x;
-    cb[j] = e.y;
-    hi = max(hi, ck[j]);
-    lo = v ? min(lo, ck[j]) : lo;
-  }
-  __syncwarp();                         // every lane holds its old entries before the list is rewritten
+  constexpr int R = 4;
+  uint32_t r[R][KPL], ck[R][2], cb[R][2];
+  uint32_t hi[R], lo[R];
+  int np[R];
   const int n_seg = j_hi > j_lo ? j_hi - j_lo : 0;
-  const int total = np + n_seg;
-  const int need = kprime < total ? kprime : total;
-  if (need <= 0) return 0;
-  uint32_t vth = 0u;                    // need == total: everything with a key (> 0) stays
-  int r_eq = 0;
-  if (need < total) {
-    hi = __reduce_max_sync(full, hi);
-    lo = __reduce_min_sync(full, lo);
-    vth = hi;
-    r_eq = need;                        // all keys equal: the `need` lowest blocks win
-    const uint32_t diff = hi ^ lo;
-    if (diff != 0u) {
-      const int top = 31 - __clz(diff);
-      uint32_t prefix = (top == 31) ? 0u : (hi & ~((2u << top) - 1u));
-      bool exact = false;
-      for (int bit = top; bit >= 0; --bit) {
-        const uint32_t c = prefix | (1u << bit);
-        int cnt = (ck[0] >= c ? 1 : 0) + (ck[1] >= c ? 1 : 0);
 #pragma unroll
-        for (int j = 0; j < KPL; ++j) cnt += (r[j] >= c) ? 1 : 0;
-        cnt = __reduce_add_sync(full, cnt);
-        if (cnt >= need) prefix = c;
-        if (cnt == need) { exact = true; break; }
-      }
-      if (exact) {
-        vth = prefix - 1u;
-        r_eq = 0;
-      } else {
-        vth = prefix;
-        int cgt = (ck[0] > vth ? 1 : 0) + (ck[1] > vth ? 1 : 0);
+  for (int a = 0; a < R; ++a) {
+    np[a] = np4[a];
+    hi[a] = 0u;
+    lo[a] = 0xffffffffu;
 #pragma unroll
-        for (int j = 0; j < KPL; ++j) cgt += (r[j] > vth) ? 1 : 0;
-        cgt = __reduce_add_sync(full, cgt);
-        r_eq = need - cgt;
-      }
-    }
-  }
-  int base = 0, eq_seen = 0;
-  const unsigned lt = (1u << lane) - 1u;
-#pragma unroll
-  for (int j = 0; j < 2; ++j) {         // carried entries first: they are the lower block indices
-    if (j * 32 < np) {
-      const bool valid = j * 32 + lane < np;
-      const bool gt = valid && ck[j] > vth;
-      const bool eq = valid && ck[j] == vth && r_eq > 0;
-      const unsigned be = __ballot_sync(full, eq);
-      const bool take = gt || (eq && (eq_seen + __popc(be & lt) < r_eq));
-      const unsigned bsel = __ballot_sync(full, take);
-      if (take) list[base + __popc(bsel & lt)] = make_uint2(ck[j], cb[j]);
-      base += __popc(bsel);
-      eq_seen += __popc(be);
-    }
-  }
-#pragma unroll
-  for (int j = 0; j < KPL; ++j) {
-    if (j * 32 < j_hi) {
+    for (int j = 0; j < KPL; ++j) {
       const int i = j * 32 + lane;
-      const bool valid = i >= j_lo && i < j_hi;
-      const bool gt = valid && r[j] > vth;
-      const bool eq = valid && r[j] == vth && r_eq > 0;
-      const unsigned be = __ballot_sync(full, eq);
-      const bool take = gt || (eq && (eq_seen + __popc(be & lt) < r_eq));
-      const unsigned bsel = __ballot_sync(full, take);
-      if (take) list[base + __popc(bsel & lt)] = make_uint2(r[j], static_cast<uint32_t>(blk0 + i));
-      base += __popc(bsel);
-      eq_seen += __popc(be);
+      const bool v = i >= j_lo && i < j_hi;
+      r[a][j] = v ? keys0[a * seg + i] : 0u;
+      hi[a] = max(hi[a], r[a][j]);
+      lo[a] = v ? min(lo[a], r[a][j]) : lo[a];
+    }
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+      const int i = j * 32 + lane;
+      const bool v = i < np[a];
+      const uint2 e = v ? list0[a * kcap + i] : make_uint2(0u, 0u);
+      ck[a][j] = e.x;
+      cb[a][j] = e.y;
+      hi[a] = max(hi[a], ck[a][j]);
+      lo[a] = v ? min(lo[a], ck[a][j]) : lo[a];
     }
   }
   __syncwarp();
-  return need;
+  uint32_t vth[R], prefix[R];
+  int r_eq[R], need[R], top[R];
+  bool open[R];                          // bisection still running for this row
+  int top_max = -1;
+#pragma unroll
+  for (int a = 0; a < R; ++a) {
+    const int total = np[a] + n_seg;
+    need[a] = kprime < total ? kprime : total;
+    vth[a] = 0u;
+    r_eq[a] = 0;
+    open[a] = false;
+    top[a] = -1;
+    prefix[a] = 0u;
+    if (need[a] > 0 && need[a] < total) {
+      hi[a] = __reduce_max_sync(full, hi[a]);
+      lo[a] = __reduce_min_sync(full, lo[a]);
+      vth[a] = hi[a];
+      r_eq[a] = need[a];
+      const uint32_t diff = hi[a] ^ lo[a];
+      if (diff != 0u) {
+        top[a] = 31 - __clz(diff);
+        prefix[a] = (top[a] == 31) ? 0u : (hi[a] & ~((2u << top[a]) - 1u));
+        open[a] = true;
+        top_max = top[a] > top_max ? top[a] : top_max;
+      }
+    }
+  }
+  bool exact[R] = {false, false, false, false};
+  for (int bit = top_max; bit >= 0; --bit) {
+    int cnt[R];
+#pragma unroll
+    for (int a = 0; a < R; ++a) {
+      const uint32_t c = prefix[a] | (1u << bit);
+      int n = (ck[a][0] >= c ? 1 : 0) + (ck[a][1] >= c ? 1 : 0);
+#pragma unroll
+      for (int j = 0; j < KPL; ++j) n += (r[a][j] >= c) ? 1 : 0;
+      cnt[a] = n;
+    }
+#pragma unroll
+    for (int a = 0; a < R; ++a) cnt[a] = __reduce_add_sync(full, cnt[a]);
+    bool any_open = false;
+#pragma unroll
+    for (int a = 0; a < R; ++a) {
+      if (open[a] && bit <= top[a]) {
+        if (cnt[a] >= need[a]) prefix[a] |= (1u << bit);
+        if (cnt[a] == need[a]) { exact[a] = true; open[a] = false; }
+      }
+      any_open = any_open || open[a];
+    }
+    if (!any_open) break;
+  }
+#pragma unroll
+  for (int a = 0; a < R; ++a) {
+    if (top[a] >= 0) {
+      if (exact[a]) {
+        vth[a] = prefix[a] - 1u;
+        r_eq[a] = 0;
+      } else {
+        vth[a] = prefix[a];
+        int cgt = (ck[a][0] > vth[a] ? 1 : 0) + (ck[a][1] > vth[a] ? 1 : 0);
+#pragma unroll
+        for (int j = 0; j < KPL; ++j) cgt += (r[a][j] > vth[a]) ? 1 : 0;
+        cgt = __reduce_add_sync(full, cgt);
+        r_eq[a] = need[a] - cgt;
+      }
+    }
+  }
+  const unsigned lt = (1u << lane) - 1u;
+#pragma unroll
+  for (int a = 0; a < R; ++a) {
+    if (need[a] <= 0) {
+      if (lane == 0) np4[a] = 0;
+      continue;
+    }
+    uint2* list = list0 + a * kcap;
+    int base = 0, eq_seen = 0;
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+      if (j * 32 < np[a]) {
+        const bool valid = j * 32 + lane < np[a];
+        const bool gt = valid && ck[a][j] > vth[a];
+        const bool eq = valid && ck[a][j] == vth[a] && r_eq[a] > 0;
+        const unsigned be = __ballot_sync(full, eq);
+        const bool take = gt || (eq && (eq_seen + __popc(be & lt) < r_eq[a]));
+        const unsigned bsel = __ballot_sync(full, take);
+        if (take) list[base + __popc(bsel & lt)] = make_uint2(ck[a][j], cb[a][j]);
+        base += __popc(bsel);
+        eq_seen += __popc(be);
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < KPL; ++j) {
+      if (j * 32 < j_hi) {
+        const int i = j * 32 + lane;
+        const bool valid = i >= j_lo && i < j_hi;
+        const bool gt = valid && r[a][j] > vth[a];
+        const bool eq = valid && r[a][j] == vth[a] && r_eq[a] > 0;
+        const unsigned be = __ballot_sync(full, eq);
+        const bool take = gt || (eq && (eq_seen + __popc(be & lt) < r_eq[a]));
+        const unsigned bsel = __ballot_sync(full, take);
+        if (take) list[base + __popc(bsel & lt)] = make_uint2(r[a][j], static_cast<uint32_t>(blk0 + i));
+        base += __popc(bsel);
+        eq_seen += __popc(be);
+      }
+    }
+    if (lane == 0) np4[a] = static_cast<int16_t>(need[a]);
+  }
+  __syncwarp();
 }
 
 template <int D, int BN, bool QUEST>
@@ -336,18 +384,13 @@ rowsel_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
           j_hi = j_hi > p.seg ? p.seg : j_hi;
           bar128();
           if (kprime > 0) {
-            for (int r = 0; r < C::RPW; ++r) {
+            for (int r = 0; r < C::RPW; r += 4) {       // four rows per call: independent bisection chains
               const int row = warp * C::RPW + r;
               const uint32_t* keys = sc + row * p.seg;
               uint2* list = lists + row * p.kcap;
-              const int n0 = np[r];
-              int n1;
-              if (p.seg == 512) n1 = row_merge<16>(keys, j_lo, j_hi, blk0, list, n0, kprime, lane);
-              else if (p.seg == 256) n1 = row_merge<8>(keys, j_lo, j_hi, blk0, list, n0, kprime, lane);
-              else n1 = row_merge<4>(keys, j_lo, j_hi, blk0, list, n0, kprime, lane);
-              __syncwarp();
-              if (lane == 0) np[r] = static_cast<int16_t>(n1);
-              __syncwarp();
+              if (p.seg == 512) row_merge4<16>(keys, p.seg, j_lo, j_hi, blk0, list, p.kcap, np + r, kprime, lane);
+              else if (p.seg == 256) row_merge4<8>(keys, p.seg, j_lo, j_hi, blk0, list, p.kcap, np + r, kprime, lane);
+              else row_merge4<4>(keys, p.seg, j_lo, j_hi, blk0, list, p.kcap, np + r, kprime, lane);
             }
           }
           bar128();
