@@ -923,3 +923,50 @@ def test_transposed_attention_variant(bsa, name, policy):
     Lg = lse[0].cpu().numpy().reshape(H, T, cfg.block)
     compare_attn(np.stack([Og[h, t] for t, h in pairs]), ref, f"transposed {name}/{policy}")
     np.testing.assert_allclose(np.stack([Lg[h, t] for t, h in pairs]), ref_lse, rtol=0, atol=3e-3)
+
+
+# ---- tiles with more than 4097 visible blocks ------------------------------------------
+def test_select_more_than_4096_blocks(bsa):
+    """N_B = 4224 (270K tokens at block 64): the register path of the selection holds 4096 keys per warp;
+    later tiles take the shared-memory bisection.  Round 1 silently ignored blocks above 4096 there.
+    Sampled tiles around and beyond the switch against the oracle, both backbones, plus attention."""
+    import dataclasses
+    import torch
+    key = "C1long"
+    if key not in _CACHE:
+        cfg = dataclasses.replace(synth.CONFIGS["C1"], name=key, number=91, seqlen=4224 * 64, n_q_heads=2,
+                                  n_kv_heads=1, k_budget=16)
+        inp = synth.make_inputs(cfg)
+        _CACHE[key] = (cfg, inp, oracle.pool(inp.K, cfg.block))
+    cfg, inp, meta_np = _CACHE[key]
+    Q, K, V = _dev(inp)
+    T, H, k, NB = cfg.n_blocks, cfg.n_q_heads, cfg.k_budget, cfg.n_blocks
+    buf = bsa.bsa_build_block_meta(K, cfg.block, 3)
+    tiles = [4095, 4096, 4097, 4098, 4099, 4100, 4160, T - 2, T - 1]
+    for policy in ("router", "router_quest"):
+        r = bsa.bsa_select(Q, buf, K, cfg.block, policy, k, 0.25)
+        torch.cuda.synchronize()
+        g = _gpu_select_np(r)
+        orc = oracle.select_tiles(inp.Q, meta_np, cfg.block, policy, k, tiles, want_scores=True)
+        for i, t in enumerate(tiles):
+            cnt = int(g["kv_count"][0, t])
+            assert cnt in (k, 2 * k)
+            for h in range(H):
+                o_row = orc["idx_sorted"][i, h]
+                if not np.array_equal(g["kv_idx"][h, t, :cnt], o_row[:cnt]):
+                    check_row(g["kv_idx"][h, t], o_row, cnt, orc["tile_score"][i, h], t, NB, f"{policy} h={h} t={t}")
+                assert abs(float(g["sigma"][h, t]) - float(orc["sigma"][i, h])) <= 1e-4
+    # winners with block index > 4096 really occur on the late tiles (otherwise the test shows nothing)
+    late = oracle.select_tiles(inp.Q, meta_np, cfg.block, "router", k, [T - 1])
+    assert (late["idx_sorted"][0, :, 2:k] > 4096).any()
+    O, _ = bsa.bsa_sparse_attn_fwd(Q, K, V, r["kv_idx"], r["kv_count"], cfg.block)
+    torch.cuda.synchronize()
+    pairs = [(T - 1, 0), (4100, 1)]
+    kv_full = np.full((H, T, r["kv_idx"].shape[-1]), NB, np.int32)
+    cnt_full = np.zeros((H, T), np.int32)
+    for t, h in pairs:
+        cnt_full[h, t] = g["kv_count"][h, t]
+        kv_full[h, t] = g["kv_idx"][h, t]
+    ref, _ = oracle.attn_pairs(inp.Q, inp.K, inp.V, cfg.block, pairs, kv_full, cnt_full)
+    Og = O[0].float().cpu().numpy().reshape(H, T, cfg.block, cfg.head_dim)
+    compare_attn(np.stack([Og[h, t] for t, h in pairs]), ref, "C1long sparse")
