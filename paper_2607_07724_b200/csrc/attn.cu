@@ -44,11 +44,19 @@ struct Cfg {
   static constexpr int kOcc = (D <= 128) ? 2 : 1;  // CTAs per SM this kernel is sized for
   static constexpr int Q_BYTES = BM * D * 2;
   static constexpr int P_BYTES = BM * BN * 2;
+  // BM = 64: P never touches shared memory.  The softmax writes P(j) (bf16 pairs) over the first 32 columns
+  // of the S buffer it has just read, and PV takes its A operand from TMEM (tcgen05.mma TS form).  The
+  // kernel is bound by shared-memory bandwidth (TMA fill 32 KB + UMMA operand reads 56 KB + P 8 KB per
+  // 64 keys at 128 B/clk/SM ~ the measured 1.5 ms at C2): this removes the P store and the A reads of PV
+  // (16 of 96 KB), the generic->async proxy fence and the wait for PV(j-1) from the softmax chain, and
+  // frees 8 KB for a sixth K/V stage.
+  static constexpr bool kPTmem = (BM == 64);
+  static constexpr int kPSmem = kPTmem ? 0 : P_BYTES;
   static constexpr int KV_BYTES = BN * D * 2;
   static constexpr int kBudget = (kOcc == 2 ? 115712 : 231424) - 1024;  // barriers + list live in 1 KB
-  static constexpr int kNSraw = (kBudget - Q_BYTES - P_BYTES) / KV_BYTES;
+  static constexpr int kNSraw = (kBudget - Q_BYTES - kPSmem) / KV_BYTES;
   static constexpr int NS = kNSraw > 8 ? 8 : kNSraw;
-  static constexpr int SMEM = Q_BYTES + P_BYTES + NS * KV_BYTES + 1024;
+  static constexpr int SMEM = Q_BYTES + kPSmem + NS * KV_BYTES + 1024;
   // TMEM: S is double buffered -- columns [0,64) and [64,128) -- so that QK(j+1) can be issued and
   // retire while the softmax warps still work on S(j); O occupies columns [128, 128+D).
   static constexpr int O_COL = 2 * BN;
@@ -70,9 +78,9 @@ struct Params {
 
 // bookkeeping block at the end of dynamic shared memory
 struct alignas(8) Ctl {
-  uint64_t q_full, p_full;
+  uint64_t q_full, p_full[2];      // per P buffer (BM = 128 uses buffer 0 only)
   uint64_t s_full[2], s_free[2];   // per S buffer
-  uint64_t o_done;
+  uint64_t o_done[2];              // PV(j) done, per P buffer
   uint64_t kv_full[8], kv_empty[8];
   uint32_t tmem_base;
   int32_t n_valid;
@@ -164,7 +172,7 @@ __device__ __forceinline__ void softmax_m128(const Params& p, Ctl* ctl, uint8_t*
     m = m_new;
 
     if (j > 0) {
-      mbar_wait(smem_u32(&ctl->o_done), (j - 1) & 1);  // PV(j-1) done: P and O are ours
+      mbar_wait(smem_u32(&ctl->o_done[0]), (j - 1) & 1);  // PV(j-1) done: P and O are ours
       tc_fence_after();
       if (any) {
 #pragma unroll
@@ -188,10 +196,10 @@ __device__ __forceinline__ void softmax_m128(const Params& p, Ctl* ctl, uint8_t*
     fence_proxy_async_smem();
     tc_fence_before();
     __syncwarp();
-    if (lane == 0) mbar_arrive(smem_u32(&ctl->p_full));
+    if (lane == 0) mbar_arrive(smem_u32(&ctl->p_full[0]));
   }
   // ---- epilogue: O / l -> bf16 -> global ---------------------------------------------------------
-  mbar_wait(smem_u32(&ctl->o_done), (n_it - 1) & 1);
+  mbar_wait(smem_u32(&ctl->o_done[0]), (n_it - 1) & 1);
   tc_fence_after();
   const float inv_l = 1.0f / l;
   const bool store = qrow < p.N;
@@ -237,8 +245,6 @@ __device__ __forceinline__ void softmax_m64(const Params& p, Ctl* ctl, uint8_t* 
   const uint32_t tS = tmem + lane_base, tO = tmem + lane_base + C::O_COL;
   const float sc = p.scale_log2;
   float mA = -INFINITY, mB = -INFINITY, lA = 0.f, lB = 0.f;
-  uint8_t* prowA = p_s + rA * 128 + quad * 4;
-  uint8_t* prowB = p_s + rB * 128 + quad * 4;
   const int sw = rA & 7;  // == rB & 7
   for (int j = 0; j < n_it; ++j) {
     const int k0 = key_start(j);
@@ -249,7 +255,7 @@ __device__ __forceinline__ void softmax_m64(const Params& p, Ctl* ctl, uint8_t* 
     tmem_ld_wait();
     tc_fence_before();
     __syncwarp();
-    if (lane == 0) mbar_arrive(smem_u32(&ctl->s_free[j & 1]));
+    // (no s_free arrival: the S buffer also carries P(j); QK(j+2) waits for PV(j) instead)
 
     float xa[16], xb[16];
 #pragma unroll
@@ -312,10 +318,11 @@ __device__ __forceinline__ void softmax_m64(const Params& p, Ctl* ctl, uint8_t* 
     mA = mA_new;
     mB = mB_new;
 
-    if (j > 0) {
-      mbar_wait(smem_u32(&ctl->o_done), (j - 1) & 1);  // PV(j-1) done: P and O are ours
+    if (any && j > 0) {
+      // the rare rescale touches O: every earlier PV must be done (they complete in order)
+      mbar_wait(smem_u32(&ctl->o_done[(j - 1) & 1]), ((j - 1) >> 1) & 1);
       tc_fence_after();
-      if (any) {
+      {
 #pragma unroll
         for (int c0 = 0; c0 < D; c0 += 64) {
           uint32_t o[32];
@@ -333,21 +340,26 @@ __device__ __forceinline__ void softmax_m64(const Params& p, Ctl* ctl, uint8_t* 
         tmem_st_wait();
       }
     }
-    // P tile [64 rows x 64 keys] bf16, K-major, 128B swizzle: 16-byte chunk g of row r sits at
-    // chunk (g ^ (r & 7)); a quad's four 4-byte stores fill one chunk, the 8 rows of a store
-    // instruction hit 8 different chunks -> 32 distinct banks.
+    // P(j) -> TMEM, over columns [0, 32) of the S buffer just read: the 16x128b store writes, per 8-key
+    // group g, the bf16 pair of row rA to (lane t/4, column 4g + t%4) and that of rB to lane t/4 + 8 --
+    // the A-operand image of the accumulator fragment (sm100_ptx.cuh).
+    {
+      uint32_t pr[16];
 #pragma unroll
-    for (int g = 0; g < 8; ++g) {
-      *reinterpret_cast<uint32_t*>(prowA + ((g ^ sw) << 4)) = pa[g];
-      *reinterpret_cast<uint32_t*>(prowB + ((g ^ sw) << 4)) = pb[g];
+      for (int g = 0; g < 8; ++g) {
+        pr[2 * g] = pa[g];
+        pr[2 * g + 1] = pb[g];
+      }
+      tmem_st16x128_x8(tS + (j & 1) * BN, pr);
+      tmem_st_wait();
     }
-    fence_proxy_async_smem();
     tc_fence_before();
     __syncwarp();
-    if (lane == 0) mbar_arrive(smem_u32(&ctl->p_full));
+    // per-buffer barrier: the softmax may publish P(j+1) before the PV thread has even looked at P(j)
+    if (lane == 0) mbar_arrive(smem_u32(&ctl->p_full[j & 1]));
   }
   // ---- epilogue: O / l -> bf16 -> global ---------------------------------------------------------
-  mbar_wait(smem_u32(&ctl->o_done), (n_it - 1) & 1);
+  mbar_wait(smem_u32(&ctl->o_done[(n_it - 1) & 1]), ((n_it - 1) >> 1) & 1);
   tc_fence_after();
   lA += __shfl_xor_sync(0xffffffffu, lA, 1);
   lB += __shfl_xor_sync(0xffffffffu, lB, 1);
@@ -387,7 +399,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
   extern __shared__ __align__(1024) uint8_t smem[];
   uint8_t* q_s = smem;
   uint8_t* p_s = smem + C::Q_BYTES;
-  uint8_t* kv_s = p_s + C::P_BYTES;
+  uint8_t* kv_s = p_s + C::kPSmem;
   Ctl* ctl = reinterpret_cast<Ctl*>(kv_s + C::NS * C::KV_BYTES);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -414,8 +426,10 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
         mbar_init(smem_u32(&ctl->s_full[i]), 1);
         mbar_init(smem_u32(&ctl->s_free[i]), 4);
       }
-      mbar_init(smem_u32(&ctl->p_full), 4);
-      mbar_init(smem_u32(&ctl->o_done), 1);
+      for (int i = 0; i < 2; ++i) {
+        mbar_init(smem_u32(&ctl->p_full[i]), 4);
+        mbar_init(smem_u32(&ctl->o_done[i]), 1);
+      }
       for (int s = 0; s < C::NS; ++s) {
         mbar_init(smem_u32(&ctl->kv_full[s]), 1);
         mbar_init(smem_u32(&ctl->kv_empty[s]), 1);
@@ -552,7 +566,12 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
         auto issue_qk = [&](int i) {
           const int s = slot_k(i);
           mbar_wait(smem_u32(&ctl->kv_full[s]), (seq_k(i) / NSK) & 1);
-          if (i >= 2) mbar_wait(smem_u32(&ctl->s_free[i & 1]), ((i >> 1) & 1) ^ 1);   // softmax(i-2) read it
+          if (i >= 2) {
+            if (C::kPTmem)   // the S buffer also holds P(i-2): PV(i-2) must have consumed it
+              mbar_wait(smem_u32(&ctl->o_done[i & 1]), ((i >> 1) & 1) ^ 1);
+            else
+              mbar_wait(smem_u32(&ctl->s_free[i & 1]), ((i >> 1) & 1) ^ 1);   // softmax(i-2) read it
+          }
           tc_fence_after();
           const uint32_t k_a = kv_a + s * C::KV_BYTES;
 #pragma unroll
@@ -567,17 +586,22 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
         auto issue_pv = [&](int jj) {
           const int s = slot_v(jj);
           mbar_wait(smem_u32(&ctl->kv_full[s]), (seq_v(jj) / NSV) & 1);
-          mbar_wait(smem_u32(&ctl->p_full), jj & 1);
+          const int pb = C::kPTmem ? (jj & 1) : 0;       // o_done barrier: per S buffer when P lives there
+          mbar_wait(smem_u32(&ctl->p_full[pb]), C::kPTmem ? ((jj >> 1) & 1) : (jj & 1));
           tc_fence_after();
           const uint32_t v_a = kv_a + s * C::KV_BYTES;
 #pragma unroll
           for (int ks = 0; ks < BN / 16; ++ks) {
-            const uint64_t ad = umma_smem_desc(p_a + ks * 32, 16, 1024);
             const uint64_t bd = umma_smem_desc(v_a + ks * 2048, BN * 128, 1024);
-            umma_ss(tO, ad, bd, idesc_pv, (jj > 0) || (ks > 0));
+            if (C::kPTmem) {   // A = P(jj) from TMEM: 16 keys = 8 columns of bf16 pairs per K step
+              umma_ts(tO, tS + (jj & 1) * BN + ks * 8, bd, idesc_pv, (jj > 0) || (ks > 0));
+            } else {
+              const uint64_t ad = umma_smem_desc(p_a + ks * 32, 16, 1024);
+              umma_ss(tO, ad, bd, idesc_pv, (jj > 0) || (ks > 0));
+            }
           }
           tc_commit(smem_u32(&ctl->kv_empty[s]));
-          tc_commit(smem_u32(&ctl->o_done));
+          tc_commit(smem_u32(&ctl->o_done[pb]));
         };
         if (kSplit) {
           if (warp == 5) {
