@@ -110,6 +110,15 @@ struct BitCursor {
 };
 static_assert(sizeof(Ctl) <= 1024, "Ctl must fit the 1 KB bookkeeping area");
 
+#ifdef BSA_TRACE
+// Debug builds only (-DBSA_TRACE): clock64 stamps of one CTA, read back with bsa_debug_trace().
+// g_tr[role][iteration][stamp]: role 0 = softmax warp 0, 1 = QK thread, 2 = PV thread.
+__device__ long long g_tr[3][32][8];
+#define TR(role, it, k) do { if (trace_on && (it) < 32) g_tr[role][it][k] = clock64(); } while (0)
+#else
+#define TR(role, it, k) do { } while (0)
+#endif
+
 // ---- softmax warps, BM = 128 (dense; sparse with 128-token blocks) -------------------------------
 // Thread r owns accumulator row r (TMEM lane r, 32x32b loads).  Logits stay unscaled in registers;
 // the softmax scale is folded into one FFMA per element: p = 2^(s*scale_log2 - m).
@@ -245,14 +254,19 @@ __device__ __forceinline__ void softmax_m64(const Params& p, Ctl* ctl, uint8_t* 
   const uint32_t tS = tmem + lane_base, tO = tmem + lane_base + C::O_COL;
   const float sc = p.scale_log2;
   float mA = -INFINITY, mB = -INFINITY, lA = 0.f, lB = 0.f;
-  const int sw = rA & 7;  // == rB & 7
+#ifdef BSA_TRACE
+  const bool trace_on = blockIdx.x == gridDim.x / 2 && tid == 0;
+#endif
   for (int j = 0; j < n_it; ++j) {
     const int k0 = key_start(j);
+    TR(0, j, 0);
     mbar_wait(smem_u32(&ctl->s_full[j & 1]), (j >> 1) & 1);
     tc_fence_after();
+    TR(0, j, 1);
     uint32_t s[32];
     tmem_ld16x256_x8(tS + (j & 1) * BN, s);
     tmem_ld_wait();
+    TR(0, j, 2);
     tc_fence_before();
     __syncwarp();
     // (no s_free arrival: the S buffer also carries P(j); QK(j+2) waits for PV(j) instead)
@@ -317,6 +331,7 @@ __device__ __forceinline__ void softmax_m64(const Params& p, Ctl* ctl, uint8_t* 
     lB = lB * alphaB + (sumB2.x + sumB2.y);
     mA = mA_new;
     mB = mB_new;
+    TR(0, j, 3);
 
     if (any && j > 0) {
       // the rare rescale touches O: every earlier PV must be done (they complete in order)
@@ -353,6 +368,7 @@ __device__ __forceinline__ void softmax_m64(const Params& p, Ctl* ctl, uint8_t* 
       tmem_st16x128_x8(tS + (j & 1) * BN, pr);
       tmem_st_wait();
     }
+    TR(0, j, 4);
     tc_fence_before();
     __syncwarp();
     // per-buffer barrier: the softmax may publish P(j+1) before the PV thread has even looked at P(j)
@@ -563,9 +579,14 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
         constexpr uint32_t idesc_pv = umma_idesc_bf16(BM, D, 0, 1);
         const uint32_t tS = tmem, tO = tmem + C::O_COL;
         const uint32_t q_a = smem_u32(q_s), p_a = smem_u32(p_s), kv_a = smem_u32(kv_s);
+#ifdef BSA_TRACE
+        const bool trace_on = blockIdx.x == gridDim.x / 2;
+#endif
         auto issue_qk = [&](int i) {
           const int s = slot_k(i);
+          TR(1, i, 0);
           mbar_wait(smem_u32(&ctl->kv_full[s]), (seq_k(i) / NSK) & 1);
+          TR(1, i, 1);
           if (i >= 2) {
             if (C::kPTmem)   // the S buffer also holds P(i-2): PV(i-2) must have consumed it
               mbar_wait(smem_u32(&ctl->o_done[i & 1]), ((i >> 1) & 1) ^ 1);
@@ -573,6 +594,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
               mbar_wait(smem_u32(&ctl->s_free[i & 1]), ((i >> 1) & 1) ^ 1);   // softmax(i-2) read it
           }
           tc_fence_after();
+          TR(1, i, 2);
           const uint32_t k_a = kv_a + s * C::KV_BYTES;
 #pragma unroll
           for (int ks = 0; ks < D / 16; ++ks) {
@@ -582,13 +604,17 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
           }
           tc_commit(smem_u32(&ctl->kv_empty[s]));
           tc_commit(smem_u32(&ctl->s_full[i & 1]));
+          TR(1, i, 3);
         };
         auto issue_pv = [&](int jj) {
           const int s = slot_v(jj);
+          TR(2, jj, 0);
           mbar_wait(smem_u32(&ctl->kv_full[s]), (seq_v(jj) / NSV) & 1);
+          TR(2, jj, 1);
           const int pb = C::kPTmem ? (jj & 1) : 0;       // o_done barrier: per S buffer when P lives there
           mbar_wait(smem_u32(&ctl->p_full[pb]), C::kPTmem ? ((jj >> 1) & 1) : (jj & 1));
           tc_fence_after();
+          TR(2, jj, 2);
           const uint32_t v_a = kv_a + s * C::KV_BYTES;
 #pragma unroll
           for (int ks = 0; ks < BN / 16; ++ks) {
@@ -602,6 +628,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
           }
           tc_commit(smem_u32(&ctl->kv_empty[s]));
           tc_commit(smem_u32(&ctl->o_done[pb]));
+          TR(2, jj, 3);
         };
         if (kSplit) {
           if (warp == 5) {
@@ -708,5 +735,11 @@ bsa_status launch_attn(const Dims& S, const void* Q, const void* K, const void* 
   }
   return fail(BSA_ERR_UNSUPPORTED, "attn: unsupported head_dim %d / block %d", S.d, S.Bn);
 }
+
+#ifdef BSA_TRACE
+extern "C" int bsa_debug_trace(long long* host) {
+  return static_cast<int>(cudaMemcpyFromSymbol(host, g_tr, sizeof(g_tr)));
+}
+#endif
 
 }  // namespace bsa
