@@ -4,8 +4,9 @@
 // (L45, L156) used as the "x dense" denominator.
 //
 // One CTA per (Q tile, head, batch); 7 warps:
-//   warps 0-3  softmax: tcgen05.ld of S, fp32 online softmax in base 2, P (bf16) -> shared memory,
-//              lazy rescale of the O accumulator in TMEM, final normalisation and store
+//   warps 0-3  softmax: tcgen05.ld of S, fp32 online softmax in base 2, P (bf16) -> shared memory
+//              (BM = 128) or back into TMEM over the S buffer just read (BM = 64: PV then takes its A
+//              operand from TMEM), lazy rescale of the O accumulator in TMEM, final normalisation and store
 //   warp 4     TMA producer: Q once, then K and V 64-key sub-blocks through a ring of stages; the
 //              row coordinate of each load is kv_idx * block ("gather" = ordinary tiled TMA loads)
 //   warp 5     one thread issues tcgen05.mma: S = Q K^T (both K-major, 128B swizzle) into TMEM and,
