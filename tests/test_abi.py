@@ -113,3 +113,50 @@ def test_select_argument_validation(lib):
                                    None) == 1              # NULL kv_idx
     assert lib.bsa_sparse_attn_fwd(ctypes.byref(s), p + 2, p, p, p, None, 4, ctypes.c_float(0), p, None,
                                    None) == 1              # misaligned Q
+
+
+def test_round2_entry_points_validate_before_any_launch(lib):
+    """bsa_select_diag, the varlen calls and the per-row bitmap calls: host-side validation only."""
+    from paper_2607_07724_b200 import binding
+    s = _shape(binding)
+    buf = ctypes.create_string_buffer(4096)
+    p = (ctypes.addressof(buf) + 255) // 256 * 256
+    dbl = ctypes.c_double
+    # diagnostics: a NULL diag struct, a NULL member and a NULL tau are refused
+    sel = lambda diag, tau: lib.bsa_select_diag(ctypes.byref(s), p, p, 1, 4, dbl(0.25), p, p, p, p, p, tau,
+                                                diag, None, 0, None)
+    assert sel(None, p) == 1
+    d = binding.BsaDiagOut(p, p, p, p, p, None)
+    assert sel(ctypes.byref(d), p) == 1
+    d = binding.BsaDiagOut(p, p, p, p, p, p)
+    assert sel(ctypes.byref(d), None) == 1
+    assert b"diagnostics" in lib.bsa_last_error()
+    # per-row bitmap: policy must be a backbone (TOPK / QUEST), 3 <= k_row <= 64
+    rows = lambda pol, k: lib.bsa_select_rows_bitmap(ctypes.byref(s), p, p, pol, k, p, p, None)
+    assert rows(1, 8) == 1 and rows(3, 8) == 1            # router policies have no per-row meaning
+    assert rows(0, 2) == 1                                # k_row < 3
+    assert rows(2, 65) == 2                               # BSA_ERR_UNSUPPORTED
+    assert lib.bsa_bitmap_words(ctypes.byref(s)) == (s.seqlen // s.block + 31) // 32
+    assert lib.bsa_sparse_attn_fwd_bitmap(ctypes.byref(s), p, p, p, None, ctypes.c_float(0), p, None, None) == 1
+    # varlen: cu_seqlens must run from 0 to seqlen in multiples of block, batch must be 1
+    i32 = ctypes.c_int32
+    cu = lambda *v: (i32 * len(v))(*v)
+    N = s.seqlen
+    ok = cu(0, N // 2, N // 2, N)                          # an empty sequence is allowed
+    assert lib.bsa_block_meta_bytes_varlen(ctypes.byref(s), ok, 3, 3) > 0
+    assert lib.bsa_block_meta_bytes_varlen(ctypes.byref(s), cu(0, N // 2 + 1, N), 2, 3) == 0
+    bad = [cu(64, N), cu(0, N - 64), cu(0, 100, N), cu(0, N, N // 2)]
+    for c in bad:
+        n = len(c) - 1
+        assert lib.bsa_build_block_meta_varlen(ctypes.byref(s), c, n, p, 3, p, None) == 1, list(c)
+        assert lib.bsa_select_varlen(ctypes.byref(s), c, n, p, p, 1, 4, dbl(0.25), p, p, p, p, p, p, None) == 1
+        assert lib.bsa_dense_attn_fwd_varlen(ctypes.byref(s), c, n, p, p, p, ctypes.c_float(0), p, None, None) == 1
+    assert lib.bsa_select_varlen(ctypes.byref(s), ok, 3, p, p, 1, 4, dbl(0.25), p, p, p, None, p, p, None) == 1
+    assert lib.bsa_sparse_attn_fwd_varlen(ctypes.byref(s), ok, 3, p, p, p, None, None, 4, ctypes.c_float(0), p,
+                                          None, None) == 1
+    s2 = _shape(binding, batch=2)
+    assert lib.bsa_build_block_meta_varlen(ctypes.byref(s2), ok, 3, p, 3, p, None) == 1
+    # limits of bsa_select are argument errors, not launches
+    big = _shape(binding, seqlen=64 * 8256)
+    assert lib.bsa_select(ctypes.byref(big), p, p, 0, 4, dbl(0.2), p, p, p, p, p, p, None, 0, None) == 2
+    assert b"8192" in lib.bsa_last_error()

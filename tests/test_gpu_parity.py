@@ -212,7 +212,8 @@ def test_sparse_attention_parity_stagewise(bsa, name, policy):
     np.testing.assert_allclose(got_lse, ref_lse, rtol=0, atol=LSE_TOL)
 
 
-@pytest.mark.parametrize("name,policy,reps", [("C2", "router_quest", 60), ("C3b", "topk", 40)])
+@pytest.mark.parametrize("name,policy,reps", [("C2", "router_quest", 60), ("C3b", "topk", 40),
+                                              ("C4", "router_quest", 20), ("C5", "router", 10)])
 def test_sparse_attention_is_deterministic(bsa, name, policy, reps):
     """Repeated launches on the same inputs must give bit-identical outputs.  (A build that issued the
     QK and PV MMAs from two threads passed the parity tests but, over tens of launches at C3b/topk,
