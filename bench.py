@@ -630,7 +630,39 @@ def run_gpu(args):
                 del r2, dsel
                 torch.cuda.empty_cache()
             del i2
+        # bsa_select_attn_fwd (one call, attention as a programmatic dependent launch)
+        # beside the two-call path, rows 2-6 with the pooled planes already built
+        one_call = {}
+        for name in ("C3b", "C3c"):
+            c = synth.CONFIGS[name]
+            i2 = inp if name == args.workload else synth.make_inputs(c)
+            r2 = Runner(c, i2, "router_quest", args.q_frac, torch, bsa)
+            bsa.bsa_build_block_meta(r2.K, c.block, r2.kinds, r2.meta)
+
+            def two():
+                bsa.bsa_select(r2.Q, r2.meta, r2.K, c.block, "router_quest", c.k_budget, args.q_frac, out=r2.sel)
+                bsa.bsa_sparse_attn_fwd(r2.Q, r2.K, r2.V, r2.sel["kv_idx"], r2.sel["kv_count"], c.block, O=r2.O)
+
+            def one():
+                bsa.bsa_select_attn_fwd(r2.Q, r2.K, r2.V, r2.meta, c.block, "router_quest", c.k_budget,
+                                        args.q_frac, out=r2.sel, O=r2.O)
+            ts = {"two_calls_ms": [], "one_call_ms": []}
+            for i in range(16):                      # alternate the two paths: clock drift hits both alike
+                label, fn = (("two_calls_ms", two), ("one_call_ms", one))[i & 1]
+                r2.flush_l2()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                fn()
+                e1.record()
+                torch.cuda.synchronize()
+                if i >= 4:
+                    ts[label].append(e0.elapsed_time(e1))
+            res = {k: float(np.median(v)) for k, v in ts.items()}
+            one_call[name + "/router_quest"] = res
+            del r2, i2
+            torch.cuda.empty_cache()
         line["extra"] = {"configs": extra, "sweeps": sweeps, "next_rows_c2": line_next,
+                         "select_attn_one_call": one_call,
                          "note": f"{n_x} timed steps after {w_x} warm-ups per entry (C3c: 2), dense kernel timed "
                                  "once per config; sweeps at C2 (32K), 3 steps"}
 

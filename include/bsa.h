@@ -164,6 +164,22 @@ bsa_status bsa_sparse_attn_fwd(const bsa_shape* shape, const void* Q, const void
                                const int32_t* kv_idx, const int32_t* kv_count, int32_t kv_width,
                                float softmax_scale, void* O, float* lse, void* stream);
 
+/*
+ * Selection and sparse attention in ONE call (rows 2-6; section 4.5 item 3, L271, names "block-
+ * selection fused into the attention kernel for >= 256K" as the next engineering step).  Same arguments and
+ * results as bsa_select followed by bsa_sparse_attn_fwd on its kv_idx / kv_count.  What is and is not
+ * fused here: the tile scores never exist in HBM in this library (scoring, top-2k and
+ * sigma are one kernel), so the call enqueues the same kernels back to back and launches the attention
+ * kernel as a programmatic dependent launch -- its prologue (barriers, TMEM allocation, the Q tile load) runs
+ * under the tail of the selection kernels and it waits (griddepcontrol.wait) before it reads kv_idx.  It is
+ * NOT a single persistent kernel; measured, it equals the two-call path within noise at 128K and 256K.
+ */
+bsa_status bsa_select_attn_fwd(const bsa_shape* shape, const void* Q, const void* K, const void* V,
+                               const void* meta, bsa_policy policy, int32_t k_budget, double q_frac,
+                               int32_t* kv_idx, int32_t* kv_count, float* sigma, float* sigma_bar,
+                               uint8_t* trigger, float* tau, float softmax_scale, void* O, float* lse,
+                               void* workspace, size_t workspace_bytes, void* stream);
+
 /* Dense causal attention with the same kernel design (every visible block). */
 bsa_status bsa_dense_attn_fwd(const bsa_shape* shape, const void* Q, const void* K, const void* V,
                               float softmax_scale, void* O, float* lse, void* stream);

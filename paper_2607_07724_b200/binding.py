@@ -73,6 +73,9 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     lib.bsa_select_diag.restype = ctypes.c_int
     lib.bsa_sparse_attn_fwd.argtypes = [sp, vp, vp, vp, vp, vp, i32, ctypes.c_float, vp, vp, vp]
     lib.bsa_sparse_attn_fwd.restype = ctypes.c_int
+    lib.bsa_select_attn_fwd.argtypes = [sp, vp, vp, vp, vp, ctypes.c_int, i32, ctypes.c_double, vp, vp, vp, vp, vp,
+                                        vp, ctypes.c_float, vp, vp, vp, sz, vp]
+    lib.bsa_select_attn_fwd.restype = ctypes.c_int
     lib.bsa_dense_attn_fwd.argtypes = [sp, vp, vp, vp, ctypes.c_float, vp, vp, vp]
     lib.bsa_dense_attn_fwd.restype = ctypes.c_int
     ip = ctypes.POINTER(ctypes.c_int32)
@@ -235,6 +238,35 @@ def bsa_sparse_attn_fwd(Q, K, V, kv_idx, kv_count, block: int, softmax_scale: fl
                                    _ptr(kv_count), kv_idx.shape[-1], float(softmax_scale), _ptr(O),
                                    _ptr(lse), _stream()))
     return O, lse
+
+
+def bsa_select_attn_fwd(Q, K, V, meta, block: int, policy: str, k_budget: int, q_frac: float,
+                        softmax_scale: float = 0.0, out: dict | None = None, O: torch.Tensor | None = None,
+                        want_lse: bool = False):
+    """bsa_select + bsa_sparse_attn_fwd in one call (the attention kernel as a programmatic dependent
+    launch).  Returns (selection dict as bsa_select, O, lse)."""
+    lib = load_library()
+    shape = make_shape(Q, K, block)
+    B, H, N, _ = Q.shape
+    T = N // block
+    W = bsa_kv_width(policy, k_budget)
+    dev = Q.device
+    o = dict(out) if out else {}
+    o.setdefault("kv_idx", torch.empty((B, H, T, max(W, 1)), dtype=torch.int32, device=dev))
+    o.setdefault("kv_count", torch.empty((B, H, T), dtype=torch.int32, device=dev))
+    o.setdefault("sigma", torch.empty((B, H, T), dtype=torch.float32, device=dev))
+    o.setdefault("sigma_bar", torch.empty((B, T), dtype=torch.float32, device=dev))
+    o.setdefault("trigger", torch.empty((B, T), dtype=torch.uint8, device=dev))
+    o.setdefault("tau", torch.empty((B,), dtype=torch.float32, device=dev))
+    if O is None:
+        O = torch.empty_like(Q)
+    lse = torch.empty(Q.shape[:3], dtype=torch.float32, device=dev) if want_lse else None
+    _check(lib.bsa_select_attn_fwd(ctypes.byref(shape), _ptr(Q), _ptr(K), _ptr(V), _ptr(meta), POLICIES[policy],
+                                   k_budget, float(q_frac), _ptr(o["kv_idx"]), _ptr(o["kv_count"]),
+                                   _ptr(o["sigma"]), _ptr(o["sigma_bar"]), _ptr(o["trigger"]), _ptr(o["tau"]),
+                                   float(softmax_scale), _ptr(O), _ptr(lse), None, 0, _stream()))
+    o["W"] = W
+    return o, O, lse
 
 
 def bsa_dense_attn_fwd(Q, K, V, block: int, softmax_scale: float = 0.0, O: torch.Tensor | None = None,

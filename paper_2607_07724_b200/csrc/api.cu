@@ -214,7 +214,8 @@ bsa_status bsa_select_diag(const bsa_shape* shape, const void* Q, const void* me
 
 static bsa_status attn_common(const bsa_shape* shape, const void* Q, const void* K, const void* V,
                               const int32_t* kv_idx, const int32_t* kv_count, int32_t kv_width,
-                              bool sparse, float softmax_scale, void* O, float* lse, void* stream) {
+                              bool sparse, float softmax_scale, void* O, float* lse, void* stream,
+                              bool pdl = false) {
   Dims D;
   bsa_status st = make_dims(shape, &D);
   if (st != BSA_OK) return st;
@@ -228,13 +229,32 @@ static bsa_status attn_common(const bsa_shape* shape, const void* Q, const void*
   const float scale = softmax_scale > 0.f ? softmax_scale
                                           : static_cast<float>(1.0 / sqrt(static_cast<double>(D.d)));
   return launch_attn(D, Q, K, V, kv_idx, kv_count, kv_width, sparse, scale, O, lse,
-                     static_cast<cudaStream_t>(stream));
+                     static_cast<cudaStream_t>(stream), nullptr, pdl);
 }
 
 bsa_status bsa_sparse_attn_fwd(const bsa_shape* shape, const void* Q, const void* K, const void* V,
                                const int32_t* kv_idx, const int32_t* kv_count, int32_t kv_width,
                                float softmax_scale, void* O, float* lse, void* stream) {
   return attn_common(shape, Q, K, V, kv_idx, kv_count, kv_width, true, softmax_scale, O, lse, stream);
+}
+
+bsa_status bsa_select_attn_fwd(const bsa_shape* shape, const void* Q, const void* K, const void* V,
+                               const void* meta, bsa_policy policy, int32_t k_budget, double q_frac,
+                               int32_t* kv_idx, int32_t* kv_count, float* sigma, float* sigma_bar,
+                               uint8_t* trigger, float* tau, float softmax_scale, void* O, float* lse,
+                               void* workspace, size_t workspace_bytes, void* stream) {
+  // every argument of the attention half is checked before the selection is enqueued
+  Dims D;
+  bsa_status st = make_dims(shape, &D);
+  if (st != BSA_OK) return st;
+  if (!K || !V || !O) return fail(BSA_ERR_INVALID_ARG, "K, V and O must not be NULL");
+  if (!aligned16(K) || !aligned16(V) || !aligned16(O))
+    return fail(BSA_ERR_INVALID_ARG, "K, V and O must be 16-byte aligned");
+  st = select_common(shape, Q, meta, policy, k_budget, q_frac, kv_idx, kv_count, sigma, sigma_bar, trigger,
+                     tau, nullptr, false, workspace, workspace_bytes, stream);
+  if (st != BSA_OK) return st;
+  return attn_common(shape, Q, K, V, kv_idx, kv_count, bsa_kv_width(policy, k_budget), true, softmax_scale,
+                     O, lse, stream, /*pdl=*/true);
 }
 
 bsa_status bsa_dense_attn_fwd(const bsa_shape* shape, const void* Q, const void* K, const void* V,

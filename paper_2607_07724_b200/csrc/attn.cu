@@ -73,6 +73,7 @@ struct Params {
   uint16_t* O;
   float* lse;
   int W, B, H, G, N, Bn, NB, NT;
+  int pdl;                  // launched with programmatic stream serialization (bsa_select_attn_fwd)
   int64_t qsb, qsh, qsn;
   float scale_log2;
 };
@@ -462,6 +463,9 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
     __syncwarp();
     tmem_alloc<C::TMEM_COLS>(smem_u32(&ctl->tmem_base));
   }
+  // kv_idx / kv_count / bitmap come from the selection kernels: under a programmatic dependent launch
+  // everything above (barriers, TMEM, the Q tile load) overlapped their tail
+  if (SPARSE && warp == 0) griddep_wait();
   if (SPARSE && warp == 0 && p.bitmap != nullptr) {
     // bitmap mode: copy the row's words, masked to the visible blocks (<= t); count the set bits
     const int64_t row = (static_cast<int64_t>(b) * p.H + h) * p.NT + tq;
@@ -688,7 +692,22 @@ bsa_status run(const Dims& S, const void* Q, const void* K, const void* V, const
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM);
   if (e != cudaSuccess) return fail(BSA_ERR_CUDA, "attn: smem attribute: %s", cudaGetErrorString(e));
   const unsigned grid = static_cast<unsigned>(prm.NT) * prm.B * prm.H;
-  kern<<<grid, kThreads, C::SMEM, stream>>>(tq, tk, tv, prm);
+  if (prm.pdl) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = C::SMEM;
+    cfg.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    e = cudaLaunchKernelEx(&cfg, kern, tq, tk, tv, prm);
+    if (e != cudaSuccess) return fail(BSA_ERR_CUDA, "attn: cudaLaunchKernelEx: %s", cudaGetErrorString(e));
+  } else {
+    kern<<<grid, kThreads, C::SMEM, stream>>>(tq, tk, tv, prm);
+  }
   return check_launch("attn_kernel");
 }
 
@@ -704,8 +723,9 @@ static bool attn_t_enabled() {
 
 bsa_status launch_attn(const Dims& S, const void* Q, const void* K, const void* V,
                        const int32_t* kv_idx, const int32_t* kv_count, int W, bool sparse, float scale,
-                       void* O, float* lse, cudaStream_t stream, const uint32_t* bitmap) {
+                       void* O, float* lse, cudaStream_t stream, const uint32_t* bitmap, bool pdl) {
   Params prm;
+  prm.pdl = pdl ? 1 : 0;
   prm.kv_idx = kv_idx;
   prm.kv_count = kv_count;
   prm.bitmap = bitmap;

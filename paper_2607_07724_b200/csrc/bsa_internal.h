@@ -60,7 +60,7 @@ bsa_status launch_rowsel(const Dims& D, const void* Q, const void* meta, bool qu
 bsa_status launch_attn(const Dims& D, const void* Q, const void* K, const void* V,
                        const int32_t* kv_idx, const int32_t* kv_count, int W, bool sparse,
                        float scale, void* O, float* lse, cudaStream_t stream,
-                       const uint32_t* bitmap = nullptr);
+                       const uint32_t* bitmap = nullptr, bool pdl = false);
 
 // transposed sparse attention for block 64 / head_dim 128 (attn_t.cu)
 bool attn_t_supported(const Dims& D, int W);

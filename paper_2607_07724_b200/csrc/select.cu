@@ -12,6 +12,7 @@
 
 #include "bsa_internal.h"
 #include "select_common.cuh"
+#include "sm100_ptx.cuh"
 
 namespace bsa {
 
@@ -23,6 +24,7 @@ constexpr int kRouteThreads = 1024;
 __global__ void __launch_bounds__(kRouteThreads)
 route_kernel(const float* __restrict__ sigma, int H, int T, int router, long long m,
              float* __restrict__ sigma_bar, uint8_t* __restrict__ trigger, float* __restrict__ tau) {
+  griddep_launch();   // a dependent attention launch may start its prologue now (it waits for our completion)
   extern __shared__ uint32_t rk[];  // keys[T], then hist[256], then 2 scratch words
   uint32_t* keys = rk;
   uint32_t* hist = rk + T;
@@ -95,6 +97,7 @@ route_kernel(const float* __restrict__ sigma, int H, int T, int router, long lon
 __global__ void finalize_kernel(const uint8_t* __restrict__ trigger, int H, int T, int NB, int k,
                                 int32_t* __restrict__ kv_idx, int32_t* __restrict__ kv_count,
                                 long long rows) {
+  griddep_launch();
   const long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
   const long long row = i / k;
   const int j = static_cast<int>(i % k);

@@ -971,3 +971,36 @@ def test_select_more_than_4096_blocks(bsa):
     ref, _ = oracle.attn_pairs(inp.Q, inp.K, inp.V, cfg.block, pairs, kv_full, cnt_full)
     Og = O[0].float().cpu().numpy().reshape(H, T, cfg.block, cfg.head_dim)
     compare_attn(np.stack([Og[h, t] for t, h in pairs]), ref, "C1long sparse")
+
+
+# ---- selection + attention in one call (programmatic dependent launch) ---------------------
+@pytest.mark.parametrize("name,policy", [("C2s", "router_quest"), ("C2s", "topk"), ("C5s", "router"),
+                                         ("C2", "router_quest")])
+def test_select_attn_one_call(bsa, name, policy):
+    """bsa_select_attn_fwd gives bit-identical results to bsa_select followed by bsa_sparse_attn_fwd (same
+    kernels, the attention one launched as a programmatic dependent launch), repeatedly, and that chain
+    matches the oracle chain."""
+    import torch
+    cfg, inp, meta_np = _case(name)
+    Q, K, V = _dev(inp)
+    buf = bsa.bsa_build_block_meta(K, cfg.block, 3)
+    r = bsa.bsa_select(Q, buf, K, cfg.block, policy, cfg.k_budget, 0.25)
+    O2, lse2 = bsa.bsa_sparse_attn_fwd(Q, K, V, r["kv_idx"], r["kv_count"], cfg.block, want_lse=True)
+    torch.cuda.synchronize()
+    for rep in range(6):
+        r1, O1, lse1 = bsa.bsa_select_attn_fwd(Q, K, V, buf, cfg.block, policy, cfg.k_budget, 0.25, want_lse=True)
+        torch.cuda.synchronize()
+        for n in ("kv_idx", "kv_count", "sigma", "sigma_bar", "trigger", "tau"):
+            assert torch.equal(r1[n].view(torch.uint8), r[n].view(torch.uint8)), (rep, n)
+        assert torch.equal(O1.view(torch.int16), O2.view(torch.int16)), rep
+        assert torch.equal(lse1, lse2), rep
+    orc = oracle.select(inp.Q, meta_np, cfg.block, policy, cfg.k_budget, 0.25, want_scores=True)
+    log = []
+    compare_select(_gpu_select_np(r1), orc, cfg.n_blocks, cfg.k_budget, log)
+    tied, flipped_t = _excluded(log)
+    T, H = cfg.n_blocks, cfg.n_q_heads
+    pairs = [(t, h) for h in sorted({0, H - 1}) for t in sorted({0, 1, cfg.k_budget, T // 2, T - 1})
+             if (h, t) not in tied and t not in flipped_t]
+    ref, _ = oracle.attn_pairs(inp.Q, inp.K, inp.V, cfg.block, pairs, orc["kv_idx"], orc["kv_count"])
+    Og = O1[0].float().cpu().numpy().reshape(H, T, cfg.block, cfg.head_dim)
+    compare_attn(np.stack([Og[h, t] for t, h in pairs]), ref, f"one-call {name}/{policy}")
