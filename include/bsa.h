@@ -13,7 +13,8 @@
  * Conventions
  *   - Every pointer named Q/K/V/O/meta/kv_idx/kv_count/sigma/sigma_bar/trigger/tau/lse/workspace is a
  *     DEVICE pointer owned by the caller; the library allocates no device memory and keeps no state
- *     between calls.  `shape` is a HOST pointer.  `stream` is a cudaStream_t passed as void*.
+ *     between calls (bsa_select_static is the one exception: a static device array, see there).
+ *     `shape` is a HOST pointer.  `stream` is a cudaStream_t passed as void*.
  *   - Every call only enqueues work on `stream`; it never synchronises and never touches the
  *     default stream.
  *   - Argument checks run on the host before any launch: BSA_ERR_INVALID_ARG, BSA_ERR_UNSUPPORTED and
@@ -120,6 +121,27 @@ bsa_status bsa_select(const bsa_shape* shape, const void* Q, const void* meta, b
                       int32_t k_budget, double q_frac, int32_t* kv_idx, int32_t* kv_count,
                       float* sigma, float* sigma_bar, uint8_t* trigger, float* tau, void* workspace,
                       size_t workspace_bytes, void* stream);
+
+/*
+ * bsa_select for callers that cannot allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): same selection, same kernels and bit-identical kv_idx / kv_count /
+ * sigma / tau as bsa_select, but the per-tile scratch (sigma_bar [B,Q_t] fp32 and trigger [B,Q_t] u8, Eq.12 /
+ * Eq.5) lives in a static __device__ array inside the library instead of caller memory.  The call allocates
+ * nothing (no cudaMalloc / cudaFree, no allocating library routine) and takes no workspace.
+ *   Limit : batch * Q_t <= BSA_STATIC_MAX_TILES; beyond it BSA_ERR_UNSUPPORTED, nothing enqueued.  The other
+ *           limits and errors are those of bsa_select.
+ *   Cost  : every GPU that loads libbsa holds the array (82 176 bytes) until the process exits.
+ *   State : all calls on a device share the one array and it keeps the last call's sigma_bar / trigger; a call
+ *           needs none of it zeroed (it overwrites what it reads).  Two bsa_select_static calls that may
+ *           overlap on the GPU (different streams, or graphs replayed concurrently) RACE on it: order them.
+ *   Set-up: the first call on a device resolves the array's device address (cudaGetSymbolAddress, once per
+ *           device, cached); make that first call outside stream capture.
+ * sigma_bar and trigger are not returned; callers that want them use bsa_select.
+ */
+#define BSA_STATIC_MAX_TILES 16384
+bsa_status bsa_select_static(const bsa_shape* shape, const void* Q, const void* meta, bsa_policy policy,
+                             int32_t k_budget, double q_frac, int32_t* kv_idx, int32_t* kv_count,
+                             float* sigma, float* tau, void* stream);
 
 /*
  * D.4 diagnostics (App. D.4; Eq.18; (A1)/(A2) L431-432), computed

@@ -19,6 +19,7 @@ BSA_DIAG_SUMMARY_LEN = 16
 DIAG_SUMMARY = ("n", "r_bar", "cv_r", "sigma_q", "gamma_q", "band_mass", "d2_q10", "d2_q50", "tau_hat",
                 "zero_gap_frac", "g_q40_pos", "g_q40_pos_over_tau_hat")
 BSA_RHO = 2
+BSA_STATIC_MAX_TILES = 16384
 POLICIES = {"topk": 0, "router": 1, "quest": 2, "router_quest": 3}
 STATUS = {0: "BSA_OK", 1: "BSA_ERR_INVALID_ARG", 2: "BSA_ERR_UNSUPPORTED",
           3: "BSA_ERR_WORKSPACE_TOO_SMALL", 4: "BSA_ERR_CUDA"}
@@ -68,6 +69,8 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     lib.bsa_select.argtypes = [sp, vp, vp, ctypes.c_int, i32, ctypes.c_double, vp, vp, vp, vp, vp, vp,
                                vp, sz, vp]
     lib.bsa_select.restype = ctypes.c_int
+    lib.bsa_select_static.argtypes = [sp, vp, vp, ctypes.c_int, i32, ctypes.c_double, vp, vp, vp, vp, vp]
+    lib.bsa_select_static.restype = ctypes.c_int
     lib.bsa_select_diag.argtypes = [sp, vp, vp, ctypes.c_int, i32, ctypes.c_double, vp, vp, vp, vp, vp, vp,
                                     ctypes.POINTER(BsaDiagOut), vp, sz, vp]
     lib.bsa_select_diag.restype = ctypes.c_int
@@ -220,6 +223,19 @@ def bsa_select(Q: torch.Tensor, meta: torch.Tensor, K_like: torch.Tensor, block:
         _check(lib.bsa_select(*args, _ptr(ws), ws_bytes, _stream()))
     o["W"] = W
     return o
+
+
+def bsa_select_static(Q: torch.Tensor, meta: torch.Tensor, K_like: torch.Tensor, block: int, policy: str,
+                      k_budget: int, q_frac: float, out: dict) -> dict:
+    """bsa_select_static: the selection with its scratch in the library's static device array.  The C call
+    allocates nothing, and neither does this wrapper: `out` must carry kv_idx [B,Hq,T,W] int32, kv_count
+    [B,Hq,T] int32, sigma [B,Hq,T] f32 and tau [B] f32.  Returns `out`."""
+    lib = load_library()
+    shape = make_shape(Q, K_like, block)
+    _check(lib.bsa_select_static(ctypes.byref(shape), _ptr(Q), _ptr(meta), POLICIES[policy], k_budget,
+                                 float(q_frac), _ptr(out["kv_idx"]), _ptr(out["kv_count"]), _ptr(out["sigma"]),
+                                 _ptr(out["tau"]), _stream()))
+    return out
 
 
 def bsa_sparse_attn_fwd(Q, K, V, kv_idx, kv_count, block: int, softmax_scale: float = 0.0,

@@ -1,9 +1,13 @@
 // api.cu -- the C ABI of libbsa (include/bsa.h): argument validation, meta / workspace layout,
 // dispatch to the kernels.  Nothing here touches the device except kernel launches on the caller's
-// stream; no device memory is allocated and no state is kept between calls.
+// stream; no device memory is allocated and no state is kept between calls.  The one exception is
+// bsa_select_static at the end of the file: its scratch is a file-scope __device__ array whose contents
+// survive from call to call.
 #include <math.h>
 #include <stdarg.h>
 #include <stdio.h>
+
+#include <mutex>
 
 #include "bsa_internal.h"
 
@@ -435,3 +439,62 @@ bsa_status bsa_sparse_attn_fwd_bitmap(const bsa_shape* shape, const void* Q, con
 }
 
 }  // extern "C"
+
+/* ---- bsa_select_static: selection for callers that cannot allocate (include/bsa.h) -------------------------
+ * sigma_bar [B, Q_t] fp32 and trigger [B, Q_t] u8 -- the scratch bsa_select otherwise takes from the caller's
+ * workspace -- live in this file-scope array, in the layout of the workspace route (bsa_select_workspace_bytes).
+ * Every GPU that loads libbsa holds the array until the process exits.  In host code `g_static_scratch` is a
+ * host-side stand-in, not a device address: the kernels get the pointer cudaGetSymbolAddress returns, looked
+ * up once per device with that device current. */
+static constexpr size_t kStaticScratchBytes =
+    (static_cast<size_t>(BSA_STATIC_MAX_TILES) * 4 + 255) / 256 * 256 +   // sigma_bar
+    (static_cast<size_t>(BSA_STATIC_MAX_TILES) + 255) / 256 * 256 + 256;  // trigger + the workspace slack
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
+static constexpr int kMaxDevices = 64;
+static std::mutex g_static_mu;
+static void* g_static_addr[kMaxDevices] = {nullptr};
+
+// Device address of g_static_scratch on the current device (cached per device ordinal).
+static bsa_status static_scratch_addr(void** out) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return fail(BSA_ERR_CUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
+  if (dev < 0 || dev >= kMaxDevices)
+    return fail(BSA_ERR_UNSUPPORTED, "bsa_select_static: device ordinal %d outside [0, %d)", dev, kMaxDevices);
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_addr[dev]) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_static_scratch);
+    if (e != cudaSuccess || !p)
+      return fail(BSA_ERR_CUDA, "cudaGetSymbolAddress(static scratch): %s", cudaGetErrorString(e));
+    g_static_addr[dev] = p;
+  }
+  *out = g_static_addr[dev];
+  return BSA_OK;
+}
+
+extern "C" bsa_status bsa_select_static(const bsa_shape* shape, const void* Q, const void* meta,
+                                        bsa_policy policy, int32_t k_budget, double q_frac, int32_t* kv_idx,
+                                        int32_t* kv_count, float* sigma, float* tau, void* stream) {
+  Dims D;
+  bsa_status st = make_dims(shape, &D);
+  if (st != BSA_OK) return st;
+  const size_t tiles = static_cast<size_t>(D.B) * D.NB;
+  if (tiles > static_cast<size_t>(BSA_STATIC_MAX_TILES))
+    return fail(BSA_ERR_UNSUPPORTED,
+                "bsa_select_static: batch * Q_t = %zu tiles, the static scratch holds at most %d "
+                "(use bsa_select with a caller workspace)", tiles, BSA_STATIC_MAX_TILES);
+  if (!Q || !meta || !kv_idx || !kv_count || !sigma)
+    return fail(BSA_ERR_INVALID_ARG, "Q, meta, kv_idx, kv_count and sigma must not be NULL");
+  st = check_device();
+  if (st != BSA_OK) return st;
+  void* scratch = nullptr;
+  st = static_scratch_addr(&scratch);
+  if (st != BSA_OK) return st;
+  // the workspace route of bsa_select with the static array as the workspace: the remaining argument checks
+  // run there before anything is enqueued.  Nothing in the scratch has to start at zero -- route_kernel
+  // writes every sigma_bar / trigger element of this call before finalize_kernel reads trigger.
+  return select_common(shape, Q, meta, policy, k_budget, q_frac, kv_idx, kv_count, sigma, nullptr, nullptr,
+                       tau, nullptr, false, scratch, kStaticScratchBytes, stream);
+}
