@@ -53,15 +53,34 @@ struct Cfg {
   // frees 8 KB for a sixth K/V stage.
   static constexpr bool kPTmem = (BM == 64);
   static constexpr int kPSmem = kPTmem ? 0 : P_BYTES;
+  // BM = 64, round 2b: Q lives in TMEM too.  A UMMA M = 64 accumulator occupies lanes 0-15 of each 32-lane
+  // quadrant; probed on B200: the D address of tcgen05.mma may carry a lane offset of 16, the accumulator then
+  // occupies lanes 16-31, and a TMEM A operand must sit in the SAME half as D (offset 0 with 16: "misaligned
+  // address").  So TMEM is two independent half-lane planes and the 256 columns hold twice what they held:
+  //   plane 0 (lane offset 0) : O [0, D)      | P(0) [D, D+32)        | P(1) [D+32, D+64)
+  //   plane 1 (lane offset 16): Q [0, D/2)    | S(0) [D/2, D/2+64)    | S(1) [D/2+64, D/2+128)
+  // QK = TS form with A = Q in plane 1 (no Q tile in shared memory: 16 KB fewer operand reads per block, no
+  // exposed shared-memory latency of the A operand, one more ring stage); P no longer aliases S, so QK(j+2)
+  // waits for softmax(j) to have READ S(j) instead of for PV(j).
+#ifndef BSA_Q_TMEM
+#define BSA_Q_TMEM 1
+#endif
+  static constexpr bool kQTmem = (BM == 64) && (BSA_Q_TMEM != 0);
+  static constexpr int kQSmem = kQTmem ? 0 : Q_BYTES;
   static constexpr int KV_BYTES = BN * D * 2;
   static constexpr int kBudget = (kOcc == 2 ? 115712 : 231424) - 1024;  // barriers + list live in 1 KB
-  static constexpr int kNSraw = (kBudget - Q_BYTES - kPSmem) / KV_BYTES;
+  static constexpr int kNSraw = (kBudget - kQSmem - kPSmem) / KV_BYTES;
   static constexpr int NS = kNSraw > 8 ? 8 : kNSraw;
-  static constexpr int SMEM = Q_BYTES + kPSmem + NS * KV_BYTES + 1024;
-  // TMEM: S is double buffered -- columns [0,64) and [64,128) -- so that QK(j+1) can be issued and
-  // retire while the softmax warps still work on S(j); O occupies columns [128, 128+D).
-  static constexpr int O_COL = 2 * BN;
-  static constexpr uint32_t TMEM_COLS = (O_COL + D <= 256) ? 256 : 512;
+  static constexpr int SMEM = kQSmem + kPSmem + NS * KV_BYTES + 1024;
+  // TMEM without kQTmem: S is double buffered -- columns [0,64) and [64,128) -- so that QK(j+1) can be
+  // issued and retire while the softmax warps still work on S(j); O occupies columns [128, 128+D).
+  static constexpr int S_COL = kQTmem ? D / 2 : 0;       // S(i) at S_COL + (i & 1) * BN
+  static constexpr int O_COL = kQTmem ? 0 : 2 * BN;
+  static constexpr int P_COL = kQTmem ? D : 0;           // P(j) at P_COL + (j & 1) * kPStride
+  static constexpr int kPStride = kQTmem ? 32 : BN;      // (aliased over S(j) without kQTmem)
+  static constexpr uint32_t kSLane = kQTmem ? 16u : 0u;  // lane offset of the Q / S plane
+  static constexpr int kColsUsed = kQTmem ? (D + 64 > D / 2 + 128 ? D + 64 : D / 2 + 128) : O_COL + D;
+  static constexpr uint32_t TMEM_COLS = (kColsUsed <= 256) ? 256 : 512;
   static_assert(NS >= 2 && ((BM != 64 && kOcc != 1) || NS >= 4), "not enough shared memory for a K/V ring");
 };
 
@@ -70,6 +89,7 @@ struct Params {
   const int32_t* kv_count;  // [B,H,T] or nullptr
   const uint32_t* bitmap;   // [B,H,T,nbw] block bitmap per (tile, head) (rowsel.cu), or nullptr
   int nbw;
+  const uint16_t* Q;        // BM = 64: the softmax warps copy the Q tile from global memory into TMEM
   uint16_t* O;
   float* lse;
   int W, B, H, G, N, Bn, NB, NT;
@@ -115,9 +135,11 @@ static_assert(sizeof(Ctl) <= 1024, "Ctl must fit the 1 KB bookkeeping area");
 #ifdef BSA_TRACE
 // Debug builds only (-DBSA_TRACE): clock64 stamps of one CTA, read back with bsa_debug_trace().
 // g_tr[role][iteration][stamp]: role 0 = softmax warp 0, 1 = QK thread, 2 = PV thread.
-__device__ long long g_tr[3][32][8];
+__device__ long long g_tr[4][32][8];   // role 3, slot 0: CTA-level stamps
 #define TR(role, it, k) do { if (trace_on && (it) < 32) g_tr[role][it][k] = clock64(); } while (0)
+#define TRW4(k) do { if (blockIdx.x == gridDim.x / 2 && threadIdx.x == 128) g_tr[3][2][k] = clock64(); } while (0)
 #else
+#define TRW4(k) do { } while (0)
 #define TR(role, it, k) do { } while (0)
 #endif
 
@@ -244,21 +266,56 @@ __device__ __forceinline__ void softmax_m128(const Params& p, Ctl* ctl, uint8_t*
 // t owns rows rA = 16w + t/4 and rB = rA + 8, and in every 8-column group the two columns
 // 2(t%4), 2(t%4)+1.  Row max = in-thread max + two quad shuffles; the row sum stays a per-thread
 // partial until the epilogue.
+// Q tile rows of this thread (rA, rB of the fragment layout below), loaded at kernel entry so that the
+// global-memory latency runs under the CTA's setup: qr[c][2g] / qr[c][2g+1] = the element pair
+// 64c + 8g + 2(t%4) of row rA / rB.
+template <int D>
+__device__ __forceinline__ void load_q_m64(const Params& p, int q0, int b, int h, uint32_t (&qr)[D / 64][16]) {
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int rA = warp * 16 + (lane >> 2);
+  const uint16_t* qbase = p.Q + b * p.qsb + h * p.qsh + 2 * (lane & 3);
+  const uint16_t* qA = qbase + static_cast<int64_t>(q0 + rA) * p.qsn;
+  const uint16_t* qB = qA + 8 * p.qsn;
+#pragma unroll
+  for (int c = 0; c < D / 64; ++c) {
+#pragma unroll
+    for (int g = 0; g < 8; ++g) {
+      qr[c][2 * g] = __ldg(reinterpret_cast<const uint32_t*>(qA + 64 * c + 8 * g));
+      qr[c][2 * g + 1] = __ldg(reinterpret_cast<const uint32_t*>(qB + 64 * c + 8 * g));
+    }
+  }
+}
+
 template <int D, bool SPARSE, class KeyStart>
 __device__ __forceinline__ void softmax_m64(const Params& p, Ctl* ctl, uint8_t* p_s, uint32_t tmem,
-                                            int n_it, int q0, int b, int h, KeyStart key_start) {
+                                            int n_it, int q0, int b, int h, KeyStart key_start,
+                                            const uint32_t (&qr)[D / 64][16]) {
   using C = Cfg<64, D>;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int quad = lane & 3;
   const int rA = warp * 16 + (lane >> 2), rB = rA + 8;
   const int qrA = q0 + rA, qrB = q0 + rB;
   const uint32_t lane_base = static_cast<uint32_t>(warp * 32) << 16;
-  const uint32_t tS = tmem + lane_base, tO = tmem + lane_base + C::O_COL;
+  const uint32_t tS = tmem + lane_base + (C::kSLane << 16) + C::S_COL;   // S(j) at tS + (j & 1) * BN
+  const uint32_t tO = tmem + lane_base + C::O_COL;
+  const uint32_t tP = tmem + lane_base + C::P_COL;                       // P(j) at tP + (j & 1) * kPStride
   const float sc = p.scale_log2;
   float mA = -INFINITY, mB = -INFINITY, lA = 0.f, lB = 0.f;
 #ifdef BSA_TRACE
   const bool trace_on = blockIdx.x == gridDim.x / 2 && tid == 0;
 #endif
+  if constexpr (C::kQTmem) {
+    // Q tile -> TMEM plane 1, columns [0, D/2): the A-operand image (word c of a row = elements 2c, 2c+1).
+    // The 16x128b store takes, per 8-element group g, the pair 8g + 2(t%4) of row rA and of row rB.
+    const uint32_t tQ = tmem + lane_base + (C::kSLane << 16);
+#pragma unroll
+    for (int c = 0; c < D / 64; ++c) tmem_st16x128_x8(tQ + 32 * c, qr[c]);
+    tmem_st_wait();
+    tc_fence_before();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(smem_u32(&ctl->q_full));
+  }
+  TR(3, 0, 2);
   for (int j = 0; j < n_it; ++j) {
     const int k0 = key_start(j);
     TR(0, j, 0);
@@ -271,7 +328,10 @@ __device__ __forceinline__ void softmax_m64(const Params& p, Ctl* ctl, uint8_t* 
     TR(0, j, 2);
     tc_fence_before();
     __syncwarp();
-    // (no s_free arrival: the S buffer also carries P(j); QK(j+2) waits for PV(j) instead)
+    if constexpr (C::kQTmem) {
+      if (lane == 0) mbar_arrive(smem_u32(&ctl->s_free[j & 1]));   // QK(j+2) may overwrite S(j)
+    }
+    // (without kQTmem no s_free arrival: the S buffer also carries P(j); QK(j+2) waits for PV(j) instead)
 
     float xa[16], xb[16];
 #pragma unroll
@@ -367,7 +427,14 @@ __device__ __forceinline__ void softmax_m64(const Params& p, Ctl* ctl, uint8_t* 
         pr[2 * g] = pa[g];
         pr[2 * g + 1] = pb[g];
       }
-      tmem_st16x128_x8(tS + (j & 1) * BN, pr);
+      if constexpr (C::kQTmem) {
+        // P has its own two buffers in plane 0: PV(j-2) must have consumed the one P(j) goes to
+        if (j >= 2 && !(any && j > 0)) {
+          mbar_wait(smem_u32(&ctl->o_done[j & 1]), ((j - 2) >> 1) & 1);
+          tc_fence_after();
+        }
+      }
+      tmem_st16x128_x8(tP + (j & 1) * C::kPStride, pr);
       tmem_st_wait();
     }
     TR(0, j, 4);
@@ -377,8 +444,10 @@ __device__ __forceinline__ void softmax_m64(const Params& p, Ctl* ctl, uint8_t* 
     if (lane == 0) mbar_arrive(smem_u32(&ctl->p_full[j & 1]));
   }
   // ---- epilogue: O / l -> bf16 -> global ---------------------------------------------------------
+  TR(3, 0, 3);
   mbar_wait(smem_u32(&ctl->o_done[(n_it - 1) & 1]), ((n_it - 1) >> 1) & 1);
   tc_fence_after();
+  TR(3, 0, 4);
   lA += __shfl_xor_sync(0xffffffffu, lA, 1);
   lB += __shfl_xor_sync(0xffffffffu, lB, 1);
   lA += __shfl_xor_sync(0xffffffffu, lA, 2);
@@ -406,6 +475,7 @@ __device__ __forceinline__ void softmax_m64(const Params& p, Ctl* ctl, uint8_t* 
     if (stA) lse[qrA] = (mA + log2f(lA)) * 0.6931471805599453f;
     if (stB) lse[qrB] = (mB + log2f(lB)) * 0.6931471805599453f;
   }
+  TR(3, 0, 5);
   tc_fence_before();
 }
 
@@ -416,7 +486,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
   using C = Cfg<BM, D>;
   extern __shared__ __align__(1024) uint8_t smem[];
   uint8_t* q_s = smem;
-  uint8_t* p_s = smem + C::Q_BYTES;
+  uint8_t* p_s = smem + C::kQSmem;
   uint8_t* kv_s = p_s + C::kPSmem;
   Ctl* ctl = reinterpret_cast<Ctl*>(kv_s + C::NS * C::KV_BYTES);
 
@@ -435,11 +505,35 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
   const int q0 = tq * BM;  // first query row of this tile
 
   if ((smem_u32(smem) & 1023u) != 0) __trap();
+#ifdef BSA_TRACE
+  const bool trace_on = blockIdx.x == gridDim.x / 2 && tid == 0;
+#endif
+  TR(3, 0, 0);   // CTA-level stamps (entry, setup done, Q in TMEM, loop end, last PV seen, stored)
+
+  uint32_t qreg[BM == 64 ? D / 64 : 1][16];
+  constexpr bool kListFirst = SPARSE && BM == 64 && C::kQTmem;   // warp 0 requests its kv_idx row first
+  if constexpr (BM == 64 && C::kQTmem) {
+    if (warp < 4 && !(kListFirst && warp == 0 && !p.pdl && p.bitmap == nullptr))
+      load_q_m64<D>(p, q0, b, h, qreg);   // in flight during the setup below
+  }
 
   // ---- setup ---------------------------------------------------------------------------------
+  // Early start (sparse list mode with split rings): the producer thread reads the first entry of the row
+  // itself and, if it is a visible block (then it is also the first entry of the compacted list), loads
+  // K(0) and V(0) before the list compaction and the CTA barrier -- the first QK no longer waits for a
+  // TMA round trip after the setup.  Slot 0 of each ring is used; the dedupe bitmap lives in the last slot.
+  constexpr bool kEarly = SPARSE && ((BM == 64) || (C::kOcc == 1)) && C::NS >= 4;
+  bool early = false;
   if (warp == 4) {
+    int e_blk = -1, e_cnt = 0;
+    if (kEarly && lane == 0 && p.bitmap == nullptr) {
+      if (p.pdl) griddep_wait();
+      const int64_t row = (static_cast<int64_t>(b) * p.H + h) * p.NT + tq;
+      e_blk = __ldg(p.kv_idx + row * p.W);
+      e_cnt = p.kv_count ? __ldg(p.kv_count + row) : p.W;
+    }
     if (lane == 0) {
-      mbar_init(smem_u32(&ctl->q_full), 1);
+      mbar_init(smem_u32(&ctl->q_full), C::kQTmem ? 4 : 1);
       for (int i = 0; i < 2; ++i) {
         mbar_init(smem_u32(&ctl->s_full[i]), 1);
         mbar_init(smem_u32(&ctl->s_free[i]), 4);
@@ -453,15 +547,28 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
         mbar_init(smem_u32(&ctl->kv_empty[s]), 1);
       }
       fence_mbar_init();
+      TRW4(0);
       // the Q tile does not depend on the kv_idx row: start it now, under the TMEM allocation and
       // the list compaction below (both ~1 us of latency)
-      mbar_arrive_expect_tx(smem_u32(&ctl->q_full), C::Q_BYTES);
-      tma_load_5d(smem_u32(q_s), &tmQ, smem_u32(&ctl->q_full), 0, q0, 0, h, b);
+      if constexpr (!C::kQTmem) {
+        mbar_arrive_expect_tx(smem_u32(&ctl->q_full), C::Q_BYTES);
+        tma_load_5d(smem_u32(q_s), &tmQ, smem_u32(&ctl->q_full), 0, q0, 0, h, b);
+      }
       tma_prefetch_desc(&tmK);
       tma_prefetch_desc(&tmV);
+      if (kEarly && e_cnt > 0 && e_blk >= 0 && e_blk < p.NB && e_blk <= tq) {
+        constexpr int NSK0 = (C::NS + 1) / 2;
+        early = true;
+        mbar_arrive_expect_tx(smem_u32(&ctl->kv_full[0]), C::KV_BYTES);
+        tma_load_5d(smem_u32(kv_s), &tmK, smem_u32(&ctl->kv_full[0]), 0, e_blk * p.Bn, 0, g, b);
+        mbar_arrive_expect_tx(smem_u32(&ctl->kv_full[NSK0]), C::KV_BYTES);
+        tma_load_5d(smem_u32(kv_s + NSK0 * C::KV_BYTES), &tmV, smem_u32(&ctl->kv_full[NSK0]), 0, e_blk * p.Bn, 0,
+                    g, b);
+      }
     }
     __syncwarp();
     tmem_alloc<C::TMEM_COLS>(smem_u32(&ctl->tmem_base));
+    TRW4(1);
   }
   // kv_idx / kv_count / bitmap come from the selection kernels: under a programmatic dependent launch
   // everything above (barriers, TMEM, the Q tile load) overlapped their tail
@@ -481,33 +588,58 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
     if (lane == 0) ctl->n_valid = cnt;
   } else if (SPARSE && warp == 0) {
     // compact the valid entries of this kv_idx row (sentinel >= N_B and blocks > t are skipped, A.10;
-    // a block listed more than once is attended once, like the oracle's O11)
+    // a block listed more than once is attended once, like the oracle's O11).  The whole row and its
+    // count are requested at once (one global-memory latency); duplicates are found with a bitmap of the
+    // visible blocks kept in the still unused K/V ring (N_B <= 65535 -> at most 8 KB).
     const int64_t row = (static_cast<int64_t>(b) * p.H + h) * p.NT + tq;
-    int cnt = p.kv_count ? p.kv_count[row] : p.W;
-    cnt = cnt < 0 ? 0 : (cnt > p.W ? p.W : cnt);
     const int32_t* src = p.kv_idx + row * p.W;
+    int blkv[kMaxW / 32];
+#pragma unroll
+    for (int c = 0; c < kMaxW / 32; ++c) blkv[c] = (c * 32 + lane < p.W) ? __ldg(src + c * 32 + lane) : -1;
+    int cnt = p.kv_count ? __ldg(p.kv_count + row) : p.W;
+    if constexpr (kListFirst) {
+      if (!p.pdl) load_q_m64<D>(p, q0, b, h, qreg);
+    }
+    TR(3, 1, 0);
+    uint32_t* seen = reinterpret_cast<uint32_t*>(kv_s + (C::NS - 1) * C::KV_BYTES);   // last ring slot
+    for (int i = lane; i <= (tq >> 5); i += 32) seen[i] = 0u;
+    __syncwarp();
+    TR(3, 1, 1);
+    cnt = cnt < 0 ? 0 : (cnt > p.W ? p.W : cnt);
+    TR(3, 1, 2);
     const unsigned lt = (1u << lane) - 1u;
     int base = 0;
-    for (int i0 = 0; i0 < cnt; i0 += 32) {
-      const int i = i0 + lane;
-      const int blk = (i < cnt) ? src[i] : -1;
-      bool ok = (blk >= 0) && (blk < p.NB) && (blk <= tq);
-      const unsigned same = __match_any_sync(0xffffffffu, ok ? blk : -1 - lane);
-      if (same & lt) ok = false;                         // duplicate inside this chunk: lowest lane wins
-      if (i0 > 0 && ok) {                                // duplicate of an earlier chunk
-        for (int u = 0; u < base; ++u)
-          if (ctl->list[u] == static_cast<uint16_t>(blk)) { ok = false; break; }
+#pragma unroll
+    for (int c = 0; c < kMaxW / 32; ++c) {
+      if (c * 32 < cnt) {
+        const int i = c * 32 + lane;
+        const int blk = (i < cnt) ? blkv[c] : -1;
+        const bool valid = (blk >= 0) && (blk < p.NB) && (blk <= tq);
+        // every valid entry marks its block; an entry that finds the mark already set is a duplicate
+        bool ok = valid && (atomicOr(&seen[blk >> 5], 1u << (blk & 31)) & (1u << (blk & 31))) == 0u;
+        if (__ballot_sync(0xffffffffu, ok) != __ballot_sync(0xffffffffu, valid)) {
+          // rare: some duplicate.  Which of two equal entries of this chunk won the atomic is arbitrary, so
+          // resolve it by position: the lowest lane of a block wins unless an earlier chunk listed the block.
+          const unsigned same = __match_any_sync(0xffffffffu, valid ? blk : -1 - lane);
+          ok = valid && !(same & lt);
+          if (ok) {
+            for (int u = 0; u < base; ++u)
+              if (ctl->list[u] == static_cast<uint16_t>(blk)) { ok = false; break; }
+          }
+        }
+        const unsigned bal = __ballot_sync(0xffffffffu, ok);
+        if (ok) ctl->list[base + __popc(bal & lt)] = static_cast<uint16_t>(blk);
+        base += __popc(bal);
       }
-      const unsigned bal = __ballot_sync(0xffffffffu, ok);
-      if (ok) ctl->list[base + __popc(bal & lt)] = static_cast<uint16_t>(blk);
-      base += __popc(bal);
-      __syncwarp();
     }
     if (lane == 0) ctl->n_valid = base;
+    TR(3, 1, 3);
+    fence_proxy_async_smem();   // the ring goes to the TMA (async proxy) after the CTA barrier below
   }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
+  TR(3, 0, 1);
   const uint32_t tmem = ctl->tmem_base;
 
   constexpr int SUBS = SPARSE ? (BM / BN) : 1;  // 64-key sub-blocks per selected block
@@ -564,11 +696,12 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
           mbar_arrive_expect_tx(smem_u32(&ctl->kv_full[s]), C::KV_BYTES);
           tma_load_5d(smem_u32(kv_s + s * C::KV_BYTES), tm, smem_u32(&ctl->kv_full[s]), 0, k0, 0, g, b);
         };
-        for (int i = 0; i < kAhead && i < n_it; ++i) load(&tmK, start_of(cur_a, i), slot_k(i), seq_k(i), NSK);
+        for (int i = early ? 1 : 0; i < kAhead && i < n_it; ++i)
+          load(&tmK, start_of(cur_a, i), slot_k(i), seq_k(i), NSK);
         for (int j = 0; j < n_it; ++j) {
           const int i = j + kAhead;
           if (i < n_it) load(&tmK, start_of(cur_a, i), slot_k(i), seq_k(i), NSK);
-          load(&tmV, start_of(cur_b, j), slot_v(j), seq_v(j), NSV);
+          if (!(early && j == 0)) load(&tmV, start_of(cur_b, j), slot_v(j), seq_v(j), NSV);
         }
       }
     } else if (warp == 5 || warp == 6) {
@@ -582,7 +715,8 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
       if (lane == 0 && (warp == 5 || kSplit)) {
         constexpr uint32_t idesc_qk = umma_idesc_bf16(BM, BN, 0, 0);
         constexpr uint32_t idesc_pv = umma_idesc_bf16(BM, D, 0, 1);
-        const uint32_t tS = tmem, tO = tmem + C::O_COL;
+        const uint32_t tS = tmem + (C::kSLane << 16) + C::S_COL, tO = tmem + C::O_COL;
+        const uint32_t tQ = tmem + (C::kSLane << 16), tP = tmem + C::P_COL;
         const uint32_t q_a = smem_u32(q_s), p_a = smem_u32(p_s), kv_a = smem_u32(kv_s);
 #ifdef BSA_TRACE
         const bool trace_on = blockIdx.x == gridDim.x / 2;
@@ -593,7 +727,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
           mbar_wait(smem_u32(&ctl->kv_full[s]), (seq_k(i) / NSK) & 1);
           TR(1, i, 1);
           if (i >= 2) {
-            if (C::kPTmem)   // the S buffer also holds P(i-2): PV(i-2) must have consumed it
+            if (C::kPTmem && !C::kQTmem)   // the S buffer also holds P(i-2): PV(i-2) must have consumed it
               mbar_wait(smem_u32(&ctl->o_done[i & 1]), ((i >> 1) & 1) ^ 1);
             else
               mbar_wait(smem_u32(&ctl->s_free[i & 1]), ((i >> 1) & 1) ^ 1);   // softmax(i-2) read it
@@ -603,9 +737,13 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
           const uint32_t k_a = kv_a + s * C::KV_BYTES;
 #pragma unroll
           for (int ks = 0; ks < D / 16; ++ks) {
-            const uint64_t ad = umma_smem_desc(q_a + (ks >> 2) * (BM * 128) + (ks & 3) * 32, 16, 1024);
             const uint64_t bd = umma_smem_desc(k_a + (ks >> 2) * (BN * 128) + (ks & 3) * 32, 16, 1024);
-            umma_ss(tS + (i & 1) * BN, ad, bd, idesc_qk, ks > 0);
+            if (C::kQTmem) {   // A = Q from TMEM (same half-lane plane as S): 16 elements = 8 columns per K step
+              umma_ts(tS + (i & 1) * BN, tQ + ks * 8, bd, idesc_qk, ks > 0);
+            } else {
+              const uint64_t ad = umma_smem_desc(q_a + (ks >> 2) * (BM * 128) + (ks & 3) * 32, 16, 1024);
+              umma_ss(tS + (i & 1) * BN, ad, bd, idesc_qk, ks > 0);
+            }
           }
           tc_commit(smem_u32(&ctl->kv_empty[s]));
           tc_commit(smem_u32(&ctl->s_full[i & 1]));
@@ -625,7 +763,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
           for (int ks = 0; ks < BN / 16; ++ks) {
             const uint64_t bd = umma_smem_desc(v_a + ks * 2048, BN * 128, 1024);
             if (C::kPTmem) {   // A = P(jj) from TMEM: 16 keys = 8 columns of bf16 pairs per K step
-              umma_ts(tO, tS + (jj & 1) * BN + ks * 8, bd, idesc_pv, (jj > 0) || (ks > 0));
+              umma_ts(tO, tP + (jj & 1) * C::kPStride + ks * 8, bd, idesc_pv, (jj > 0) || (ks > 0));
             } else {
               const uint64_t ad = umma_smem_desc(p_a + ks * 32, 16, 1024);
               umma_ss(tO, ad, bd, idesc_pv, (jj > 0) || (ks > 0));
@@ -654,14 +792,14 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
     } else if (warp < 4) {
       // ---- softmax warps ---------------------------------------------------------------------
       if constexpr (BM == 64) {
-        softmax_m64<D, SPARSE>(p, ctl, p_s, tmem, n_it, q0, b, h, key_start);
+        softmax_m64<D, SPARSE>(p, ctl, p_s, tmem, n_it, q0, b, h, key_start, qreg);
       } else {
         softmax_m128<D, SPARSE>(p, ctl, p_s, tmem, n_it, q0, b, h, key_start);
       }
     }
   } else if (warp < 4) {
     // nothing attended (possible only with a caller-provided kv_idx): zeros, lse = -inf
-    mbar_wait(smem_u32(&ctl->q_full), 0);   // the Q tile load must land before the CTA may exit
+    if constexpr (!C::kQTmem) mbar_wait(smem_u32(&ctl->q_full), 0);   // the Q tile load must land before the CTA may exit
     const bool active = (BM == 128) || (lane < 16);
     const int r = (BM == 128) ? tid : (warp * 16 + (lane & 15));
     const int qrow = q0 + r;
@@ -675,6 +813,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
   // ---- teardown ------------------------------------------------------------------------------
   tc_fence_before();
   __syncthreads();
+  TR(3, 0, 6);
   if (warp == 4) tmem_dealloc<C::TMEM_COLS>(tmem);
 }
 
@@ -733,6 +872,7 @@ bsa_status launch_attn(const Dims& S, const void* Q, const void* K, const void* 
   if (bitmap && S.NB > 32 * (kMaxW / 2))
     return fail(BSA_ERR_UNSUPPORTED, "bitmap attention: %d blocks per sequence, at most %d", S.NB,
                 32 * (kMaxW / 2));
+  prm.Q = static_cast<const uint16_t*>(Q);
   prm.O = static_cast<uint16_t*>(O);
   prm.lse = lse;
   prm.W = W;
