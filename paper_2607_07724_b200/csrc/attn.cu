@@ -319,7 +319,13 @@ __device__ __forceinline__ void softmax_m64(const Params& p, Ctl* ctl, uint8_t* 
   for (int j = 0; j < n_it; ++j) {
     const int k0 = key_start(j);
     TR(0, j, 0);
-    mbar_wait(smem_u32(&ctl->s_full[j & 1]), (j >> 1) & 1);
+    if (C::kQTmem && j >= 2) {
+      // S(j) ready, and PV(j-2) done so that P(j) may later overwrite P(j-2): one poll for both
+      mbar_wait2_warp(smem_u32(&ctl->s_full[j & 1]), (j >> 1) & 1, smem_u32(&ctl->o_done[j & 1]),
+                      ((j - 2) >> 1) & 1);
+    } else {
+      mbar_wait(smem_u32(&ctl->s_full[j & 1]), (j >> 1) & 1);
+    }
     tc_fence_after();
     TR(0, j, 1);
     uint32_t s[32];
@@ -382,8 +388,16 @@ __device__ __forceinline__ void softmax_m64(const Params& p, Ctl* ctl, uint8_t* 
     for (int g = 0; g < 8; ++g) {
       const float2 ta = ffma2(make_float2(xa[2 * g], xa[2 * g + 1]), sc2, nmA);
       const float2 tb = ffma2(make_float2(xb[2 * g], xb[2 * g + 1]), sc2, nmB);
+#if defined(BSA_ABL) && BSA_ABL == 1
+      const float2 ea = make_float2(ex2_approx(ta.x), fmaf(ta.y, 0.001f, 0.5f));
+      const float2 eb = make_float2(ex2_approx(tb.x), fmaf(tb.y, 0.001f, 0.5f));
+#elif defined(BSA_ABL) && BSA_ABL == 2
+      const float2 ea = make_float2(fmaf(ta.x, 0.001f, 0.5f), fmaf(ta.y, 0.001f, 0.5f));
+      const float2 eb = make_float2(fmaf(tb.x, 0.001f, 0.5f), fmaf(tb.y, 0.001f, 0.5f));
+#else
       const float2 ea = make_float2(ex2_approx(ta.x), ex2_approx(ta.y));
       const float2 eb = make_float2(ex2_approx(tb.x), ex2_approx(tb.y));
+#endif
       sumA2 = fadd2(sumA2, ea);
       sumB2 = fadd2(sumB2, eb);
       pa[g] = pack_bf16x2(ea.x, ea.y);
@@ -427,13 +441,8 @@ __device__ __forceinline__ void softmax_m64(const Params& p, Ctl* ctl, uint8_t* 
         pr[2 * g] = pa[g];
         pr[2 * g + 1] = pb[g];
       }
-      if constexpr (C::kQTmem) {
-        // P has its own two buffers in plane 0: PV(j-2) must have consumed the one P(j) goes to
-        if (j >= 2 && !(any && j > 0)) {
-          mbar_wait(smem_u32(&ctl->o_done[j & 1]), ((j - 2) >> 1) & 1);
-          tc_fence_after();
-        }
-      }
+      // (kQTmem: P has its own two buffers in plane 0; that PV(j-2) has consumed the one P(j) goes to was
+      // checked together with s_full at the top of the iteration)
       tmem_st16x128_x8(tP + (j & 1) * C::kPStride, pr);
       tmem_st_wait();
     }

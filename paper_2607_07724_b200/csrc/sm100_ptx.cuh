@@ -56,6 +56,19 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 #endif
 }
 
+// One warp waits for TWO barriers at the price of one poll: lanes 0-15 poll (bar_a, par_a), lanes 16-31
+// (bar_b, par_b), until both halves have seen their phase complete.  (A lone mbarrier poll costs a warp
+// ~100 clk even when the phase is long complete; two waits in a row were 2 x 100 clk of the softmax chain.)
+// All 32 lanes must call it.
+__device__ __forceinline__ void mbar_wait2_warp(uint32_t bar_a, uint32_t par_a, uint32_t bar_b, uint32_t par_b) {
+  const bool hi = (threadIdx.x & 16u) != 0;
+  const uint32_t bar = hi ? bar_b : bar_a, par = hi ? par_b : par_a;
+  bool done = mbar_try_wait(bar, par);
+  while (!__all_sync(0xffffffffu, done)) {
+    if (!done) done = mbar_try_wait(bar, par);
+  }
+}
+
 // Programmatic dependent launch: a kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may
 // start while its predecessor in the stream still runs; griddep_wait() blocks until that predecessor has
 // completed and its writes are visible (a no-op for an ordinary launch); griddep_launch() in the predecessor
