@@ -17,6 +17,9 @@
 #include <cuda_bf16.h>
 #include <stdlib.h>
 
+#include <atomic>
+#include <type_traits>
+
 #include "bsa_internal.h"
 #include "sm100_ptx.cuh"
 #include "tmap.h"
@@ -266,6 +269,21 @@ __device__ __forceinline__ void softmax_m128(const Params& p, Ctl* ctl, uint8_t*
 // t owns rows rA = 16w + t/4 and rB = rA + 8, and in every 8-column group the two columns
 // 2(t%4), 2(t%4)+1.  Row max = in-thread max + two quad shuffles; the row sum stays a per-thread
 // partial until the epilogue.
+// Epilogue helper for the BM = 64 fragment layout: thread q = lane % 4 of a quad holds, for every 8-column group,
+// the word (two bf16) at columns 2q, 2q+1.  Two shuffle rounds turn the words w0..w3 of four consecutive groups
+// g0..g0+3 into the complete 16 bytes of group g0 + q, so that a row leaves as 64 contiguous bytes per quad and
+// store instruction instead of 16 (32 four-byte stores per thread kept the store path busy for ~2000 clk).
+__device__ __forceinline__ uint4 quad_gather(uint32_t w0, uint32_t w1, uint32_t w2, uint32_t w3, int q) {
+  const bool odd = (q & 1) != 0, hi = (q & 2) != 0;
+  const uint32_t r01 = __shfl_xor_sync(0xffffffffu, odd ? w0 : w1, 1);
+  const uint32_t r23 = __shfl_xor_sync(0xffffffffu, odd ? w2 : w3, 1);
+  const uint32_t ax = odd ? r01 : w0, ay = odd ? w1 : r01;   // even q: group g0 (+2: bx, by), odd q: group g0 + 1 (+3)
+  const uint32_t bx = odd ? r23 : w2, by = odd ? w3 : r23;
+  const uint32_t rx = __shfl_xor_sync(0xffffffffu, hi ? ax : bx, 2);
+  const uint32_t ry = __shfl_xor_sync(0xffffffffu, hi ? ay : by, 2);
+  return hi ? make_uint4(rx, ry, bx, by) : make_uint4(ax, ay, rx, ry);
+}
+
 // Q tile rows of this thread (rA, rB of the fragment layout below), loaded at kernel entry so that the
 // global-memory latency runs under the CTA's setup: qr[c][2g] / qr[c][2g+1] = the element pair
 // 64c + 8g + 2(t%4) of row rA / rB.
@@ -826,6 +844,556 @@ attn_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUt
   if (warp == 4) tmem_dealloc<C::TMEM_COLS>(tmem);
 }
 
+
+// =================================================================================================
+// Persistent variant for 64-token blocks in list mode (round 2c).
+//
+// A clock64 trace of attn_kernel<64,128,true> at C2 showed ~10.5k clk of every CTA's 51k-86k outside
+// the steady-state loop: barrier / TMEM set-up and the kv_idx row (4.4k), the first TMA round trip
+// (2.2k), the wait for the last PV (2.0k), the epilogue (1.2k) and the teardown (0.7k) -- and a CTA that
+// is not in its loop leaves the tensor pipe to its single co-resident CTA, which alone cannot fill it.
+// Here 2 x #SM CTAs stay resident and walk through the (tile, head) items; every role runs ahead across
+// item boundaries on its own:
+//   warp 7     scheduler + list builder, one item ahead: fetches the next item from a work counter
+//              (dynamic: the items' lengths differ by 2x between routed and unrouted tiles), compacts
+//              its kv_idx row into list[n & 1]
+//   warp 4     TMA producer: keeps the K / V rings full across items
+//   warp 5 / 6 QK / PV issue; buffers and mbarrier phases are indexed by a running iteration count
+//   warps 0-3  softmax; after the last iteration of an item they fetch the NEXT item's Q tile and put it
+//              into TMEM while the last PV drains, so QK(0) of the next item runs under this item's epilogue
+// Items with an empty list are written as zeros by the softmax warps and are invisible to the other
+// roles' barriers.  Same arithmetic, in the same order, as attn_kernel: outputs are bit-identical.
+// =================================================================================================
+constexpr int kMaxWP = 128;          // widest kv_idx row of the persistent kernel (two lists fit the 1 KB block)
+constexpr int kThreadsP = 256;
+constexpr int kCounterSlots = 1024;  // work counters: one per launch in flight (a launch takes slot
+                                     // ticket % 1024 and its last CTA clears it)
+__device__ unsigned int g_work_counter[kCounterSlots];
+__device__ unsigned int g_work_done[kCounterSlots];
+
+struct alignas(8) CtlP {
+  uint64_t q_full, o_free;
+  uint64_t p_full[2], s_full[2], s_free[2], o_done[2];
+  uint64_t list_full[2], list_free[2];
+  uint64_t kv_full[8], kv_empty[8];
+  uint32_t tmem_base;
+  int32_t item[2];             // work item of list buffer b, -1 = no more work
+  int32_t n_valid[2];
+  int32_t tq[2], kvh[2], bat[2], qh[2];   // the item decoded by the scheduler warp (tile, KV head, batch, head)
+  uint16_t list[2][kMaxWP];
+};
+static_assert(sizeof(CtlP) <= 1024, "CtlP must fit the 1 KB bookkeeping area");
+
+struct ItemP {
+  int tq, g, b, h, q0;
+};
+__device__ __forceinline__ ItemP decode_item(const Params& p, int wi) {
+  ItemP it;
+  const int hi = wi % p.G;
+  wi /= p.G;
+  it.tq = p.NT - 1 - wi % p.NT;
+  wi /= p.NT;
+  const int Hkv = p.H / p.G;
+  it.g = wi % Hkv;
+  it.b = wi / Hkv;
+  it.h = it.g * p.G + hi;
+  it.q0 = it.tq * 64;
+  return it;
+}
+
+__device__ __forceinline__ ItemP read_item(const CtlP* ctl, int buf) {
+  ItemP it;
+  it.tq = ctl->tq[buf]; it.g = ctl->kvh[buf]; it.b = ctl->bat[buf]; it.h = ctl->qh[buf];
+  it.q0 = it.tq * 64;
+  return it;
+}
+
+template <int D>
+__global__ void __launch_bounds__(kThreadsP, Cfg<64, D>::kOcc)
+attn64p_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV, const Params p,
+               const int n_items, const int cslot) {
+  using C = Cfg<64, D>;
+  static_assert(C::kQTmem, "the persistent kernel keeps Q in TMEM");
+  extern __shared__ __align__(1024) uint8_t smem[];
+  uint8_t* kv_s = smem;
+  CtlP* ctl = reinterpret_cast<CtlP*>(kv_s + C::NS * C::KV_BYTES);
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  constexpr int NSK = (C::NS + 1) / 2, NSV = C::NS - NSK;
+  // Q is double buffered in plane 1 (buffer = index of the non-empty item & 1): the second copy sits in the
+  // columns the one-item kernel leaves unused, so the next item's tile can be written during this item's loop
+  constexpr uint32_t kQ1Col = (D == 256) ? 256 : 192;
+  constexpr int kQChunks = D / 32;   // 16-column (32-element) pieces of a Q tile, one per late iteration
+  if ((smem_u32(smem) & 1023u) != 0) __trap();
+
+  if (warp == 4) {
+    if (lane == 0) {
+      mbar_init(smem_u32(&ctl->q_full), 4);
+      mbar_init(smem_u32(&ctl->o_free), 4);
+      for (int i = 0; i < 2; ++i) {
+        mbar_init(smem_u32(&ctl->p_full[i]), 4);
+        mbar_init(smem_u32(&ctl->s_full[i]), 1);
+        mbar_init(smem_u32(&ctl->s_free[i]), 4);
+        mbar_init(smem_u32(&ctl->o_done[i]), 1);
+        mbar_init(smem_u32(&ctl->list_full[i]), 1);
+        mbar_init(smem_u32(&ctl->list_free[i]), 7);   // 4 softmax warps, producer, QK thread, PV thread
+      }
+      for (int s = 0; s < C::NS; ++s) {
+        mbar_init(smem_u32(&ctl->kv_full[s]), 1);
+        mbar_init(smem_u32(&ctl->kv_empty[s]), 1);
+      }
+      fence_mbar_init();
+      tma_prefetch_desc(&tmK);
+      tma_prefetch_desc(&tmV);
+    }
+    __syncwarp();
+    tmem_alloc<C::TMEM_COLS>(smem_u32(&ctl->tmem_base));
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = ctl->tmem_base;
+
+  if (warp == 7) {
+    // ---- scheduler + list builder, one item ahead of everybody else ------------------------------------
+    if (p.pdl) griddep_wait();
+    for (int n = 0;; ++n) {
+      const int buf = n & 1;
+      if (n >= 2) mbar_wait(smem_u32(&ctl->list_free[buf]), ((n - 2) >> 1) & 1);
+      int wi = 0;
+      if (lane == 0) wi = static_cast<int>(atomicAdd(&g_work_counter[cslot], 1u));
+      wi = __shfl_sync(0xffffffffu, wi, 0);
+      if (wi >= n_items) {
+        if (lane == 0) {
+          ctl->item[buf] = -1;
+          mbar_arrive(smem_u32(&ctl->list_full[buf]));
+        }
+        break;
+      }
+      const ItemP it = decode_item(p, wi);
+      const int64_t row = (static_cast<int64_t>(it.b) * p.H + it.h) * p.NT + it.tq;
+      const int32_t* src = p.kv_idx + row * p.W;
+      int blkv[kMaxWP / 32];
+#pragma unroll
+      for (int c = 0; c < kMaxWP / 32; ++c) blkv[c] = (c * 32 + lane < p.W) ? __ldg(src + c * 32 + lane) : -1;
+      int cnt = p.kv_count ? __ldg(p.kv_count + row) : p.W;
+      cnt = cnt < 0 ? 0 : (cnt > p.W ? p.W : cnt);
+      const unsigned lt = (1u << lane) - 1u;
+      uint16_t* list = ctl->list[buf];
+      int base = 0;
+#pragma unroll
+      for (int c = 0; c < kMaxWP / 32; ++c) {
+        if (c * 32 < cnt) {
+          const int i = c * 32 + lane;
+          const int blk = (i < cnt) ? blkv[c] : -1;
+          bool ok = (blk >= 0) && (blk < p.NB) && (blk <= it.tq);
+          // a block listed more than once is attended once (O11): lowest position wins
+          const unsigned same = __match_any_sync(0xffffffffu, ok ? blk : -1 - lane);
+          if (same & lt) ok = false;
+          if (c > 0 && ok) {
+            for (int u = 0; u < base; ++u)
+              if (list[u] == static_cast<uint16_t>(blk)) { ok = false; break; }
+          }
+          const unsigned bal = __ballot_sync(0xffffffffu, ok);
+          if (ok) list[base + __popc(bal & lt)] = static_cast<uint16_t>(blk);
+          base += __popc(bal);
+          __syncwarp();
+        }
+      }
+      __syncwarp();
+      if (lane == 0) {
+        ctl->item[buf] = wi;
+        ctl->n_valid[buf] = base;
+        ctl->tq[buf] = it.tq; ctl->kvh[buf] = it.g; ctl->bat[buf] = it.b; ctl->qh[buf] = it.h;
+        mbar_arrive(smem_u32(&ctl->list_full[buf]));
+      }
+    }
+  } else if (warp == 4) {
+    // ---- TMA producer: per item K(0), K(1), then [K(j+2), V(j)]; ring positions run across items --------
+    if (lane == 0) {
+      uint32_t gk = 0, gv = 0;
+      auto load = [&](const CUtensorMap* tm, int k0, int s, uint32_t use, const ItemP& it) {
+        mbar_wait(smem_u32(&ctl->kv_empty[s]), (use & 1) ^ 1);
+        mbar_arrive_expect_tx(smem_u32(&ctl->kv_full[s]), C::KV_BYTES);
+        tma_load_5d(smem_u32(kv_s + s * C::KV_BYTES), tm, smem_u32(&ctl->kv_full[s]), 0, k0, 0, it.g, it.b);
+      };
+      for (int n = 0;; ++n) {
+        const int buf = n & 1;
+        mbar_wait(smem_u32(&ctl->list_full[buf]), (n >> 1) & 1);
+        const int wi = ctl->item[buf];
+        if (wi < 0) break;
+        const ItemP it = read_item(ctl, buf);
+        const int n_it = ctl->n_valid[buf];
+        const uint16_t* list = ctl->list[buf];
+        auto ldk = [&](int i) { load(&tmK, static_cast<int>(list[i]) * 64, gk % NSK, gk / NSK, it); ++gk; };
+        auto ldv = [&](int j) { load(&tmV, static_cast<int>(list[j]) * 64, NSK + gv % NSV, gv / NSV, it); ++gv; };
+        for (int i = 0; i < 2 && i < n_it; ++i) ldk(i);
+        for (int j = 0; j < n_it; ++j) {
+          if (j + 2 < n_it) ldk(j + 2);
+          ldv(j);
+        }
+        mbar_arrive(smem_u32(&ctl->list_free[buf]));
+      }
+    }
+  } else if (warp == 5) {
+    // ---- QK issue: S(gi) = Q K^T (TS form, A = Q in TMEM plane 1) into S buffer gi & 1 ----------------------
+    if (lane == 0) {
+      constexpr uint32_t idesc_qk = umma_idesc_bf16(64, BN, 0, 0);
+      const uint32_t tS = tmem + (C::kSLane << 16) + C::S_COL, tQ = tmem + (C::kSLane << 16);
+      const uint32_t kv_a = smem_u32(kv_s);
+      uint32_t gi = 0, gk = 0, ne = 0;   // running iteration, K ring position, non-empty items so far
+      for (int n = 0;; ++n) {
+        const int buf = n & 1;
+        mbar_wait(smem_u32(&ctl->list_full[buf]), (n >> 1) & 1);
+        const int wi = ctl->item[buf];
+        const int n_it = ctl->n_valid[buf];
+        if (wi < 0) break;
+        mbar_arrive(smem_u32(&ctl->list_free[buf]));
+        if (n_it == 0) continue;
+        mbar_wait(smem_u32(&ctl->q_full), ne & 1);   // this item's Q tile is in TMEM, buffer ne & 1
+        const uint32_t tQn = tQ + (ne & 1) * kQ1Col;
+        ++ne;
+        for (int i = 0; i < n_it; ++i, ++gi, ++gk) {
+          const int s = gk % NSK;
+          mbar_wait(smem_u32(&ctl->kv_full[s]), (gk / NSK) & 1);
+          if (gi >= 2) mbar_wait(smem_u32(&ctl->s_free[gi & 1]), ((gi >> 1) & 1) ^ 1);   // softmax(gi-2) read it
+          tc_fence_after();
+          const uint32_t k_a = kv_a + s * C::KV_BYTES;
+#pragma unroll
+          for (int ks = 0; ks < D / 16; ++ks) {
+            const uint64_t bd = umma_smem_desc(k_a + (ks >> 2) * (BN * 128) + (ks & 3) * 32, 16, 1024);
+            umma_ts(tS + (gi & 1) * BN, tQn + ks * 8, bd, idesc_qk, ks > 0);
+          }
+          tc_commit(smem_u32(&ctl->kv_empty[s]));
+          tc_commit(smem_u32(&ctl->s_full[gi & 1]));
+        }
+      }
+    }
+  } else if (warp == 6) {
+    // ---- PV issue: O += P(gj) V (TS form, A = P in TMEM plane 0) -----------------------------------------------
+    if (lane == 0) {
+      constexpr uint32_t idesc_pv = umma_idesc_bf16(64, D, 0, 1);
+      const uint32_t tO = tmem + C::O_COL, tP = tmem + C::P_COL;
+      const uint32_t kv_a = smem_u32(kv_s);
+      uint32_t gj = 0, gv = 0, ne = 0;
+      for (int n = 0;; ++n) {
+        const int buf = n & 1;
+        mbar_wait(smem_u32(&ctl->list_full[buf]), (n >> 1) & 1);
+        const int wi = ctl->item[buf];
+        const int n_it = ctl->n_valid[buf];
+        if (wi < 0) break;
+        mbar_arrive(smem_u32(&ctl->list_free[buf]));
+        if (n_it == 0) continue;
+        if (ne > 0) mbar_wait(smem_u32(&ctl->o_free), (ne - 1) & 1);   // the previous item's epilogue has read O
+        ++ne;
+        for (int jj = 0; jj < n_it; ++jj, ++gj, ++gv) {
+          const int s = NSK + gv % NSV;
+          mbar_wait(smem_u32(&ctl->kv_full[s]), (gv / NSV) & 1);
+          mbar_wait(smem_u32(&ctl->p_full[gj & 1]), (gj >> 1) & 1);
+          tc_fence_after();
+          const uint32_t v_a = kv_a + s * C::KV_BYTES;
+#pragma unroll
+          for (int ks = 0; ks < BN / 16; ++ks) {
+            const uint64_t bd = umma_smem_desc(v_a + ks * 2048, BN * 128, 1024);
+            umma_ts(tO, tP + (gj & 1) * C::kPStride + ks * 8, bd, idesc_pv, (jj > 0) || (ks > 0));
+          }
+          tc_commit(smem_u32(&ctl->kv_empty[s]));
+          tc_commit(smem_u32(&ctl->o_done[gj & 1]));
+        }
+      }
+    }
+  } else if (warp < 4) {
+    // ---- softmax warps ------------------------------------------------------------------------------------------
+    const int quad = lane & 3;
+    const int rA = warp * 16 + (lane >> 2);
+    const uint32_t lane_base = static_cast<uint32_t>(warp * 32) << 16;
+    const uint32_t tS = tmem + lane_base + (C::kSLane << 16) + C::S_COL;
+    const uint32_t tQ = tmem + lane_base + (C::kSLane << 16);
+    const uint32_t tO = tmem + lane_base + C::O_COL;
+    const uint32_t tP = tmem + lane_base + C::P_COL;
+    const float sc = p.scale_log2;
+    uint32_t gj = 0, ne = 0;    // running iteration count / non-empty items so far
+    bool q_ready = false;       // the current item's Q tile was already put into TMEM during the previous item
+    auto post_q = [&]() {
+      tmem_st_wait();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(smem_u32(&ctl->q_full));
+    };
+    auto put_q = [&](const ItemP& it, uint32_t tq_dst) {   // the whole tile at once (first item, short items)
+      uint32_t qr[D / 64][16];
+      load_q_m64<D>(p, it.q0, it.b, it.h, qr);
+#pragma unroll
+      for (int c = 0; c < D / 64; ++c) tmem_st16x128_x8(tq_dst + 32 * c, qr[c]);
+      post_q();
+    };
+    for (int n = 0;; ++n) {
+      const int buf = n & 1;
+      mbar_wait(smem_u32(&ctl->list_full[buf]), (n >> 1) & 1);
+      if (ctl->item[buf] < 0) break;
+      const int n_it = ctl->n_valid[buf];
+      const int q0 = ctl->tq[buf] * 64;
+      const uint16_t* list = ctl->list[buf];
+#ifdef BSA_TRACE
+      const bool trace_on = blockIdx.x == gridDim.x / 2 && tid == 0;
+#endif
+      TR(0, n, 0);
+      if (n_it == 0) {
+        // nothing attended (possible only with a caller-provided kv_idx): zeros, lse = -inf
+        const ItemP it = read_item(ctl, buf);
+        uint16_t* orowA = p.O + it.b * p.qsb + it.h * p.qsh + static_cast<int64_t>(q0 + rA) * p.qsn + 2 * quad;
+        uint16_t* orowB = orowA + 8 * p.qsn;
+#pragma unroll
+        for (int c = 0; c < D; c += 8) {
+          *reinterpret_cast<uint32_t*>(orowA + c) = 0u;
+          *reinterpret_cast<uint32_t*>(orowB + c) = 0u;
+        }
+        if (p.lse && quad == 0) {
+          float* lse = p.lse + (static_cast<int64_t>(it.b) * p.H + it.h) * p.N + q0 + rA;
+          lse[0] = -INFINITY;
+          lse[8] = -INFINITY;
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&ctl->list_free[buf]));
+        continue;
+      }
+      if (!q_ready) put_q(read_item(ctl, buf), tQ + (ne & 1) * kQ1Col);
+      q_ready = false;
+      ++ne;
+      const uint32_t tQnext = tQ + (ne & 1) * kQ1Col;   // where the next non-empty item's tile goes
+      float mA = -INFINITY, mB = -INFINITY, lA = 0.f, lB = 0.f;
+
+      // One iteration.  PIECE: the iteration also carries a 16-column piece of the NEXT item's Q tile (8 loads
+      // at its top, one store at its end) -- the last kQChunks iterations of an item, if the scheduler has
+      // posted the next item by then.  Two instances of the body keep the pieces' registers out of the main loop.
+      auto iteration = [&](const int j, auto piece_tag, const uint16_t* qnA, const int pc) {
+        constexpr bool PIECE = decltype(piece_tag)::value;
+        const int k0 = static_cast<int>(list[j]) * 64;
+        uint32_t qn[8];
+        if constexpr (PIECE) {
+          const uint16_t* a = qnA + 32 * pc;
+          const uint16_t* bq = a + 8 * p.qsn;
+#pragma unroll
+          for (int g = 0; g < 4; ++g) {
+            qn[2 * g] = __ldg(reinterpret_cast<const uint32_t*>(a + 8 * g));
+            qn[2 * g + 1] = __ldg(reinterpret_cast<const uint32_t*>(bq + 8 * g));
+          }
+        }
+        if (gj >= 2) {
+          // S(gj) ready, and PV(gj-2) done so that P(gj) may later overwrite P(gj-2): one poll for both
+          mbar_wait2_warp(smem_u32(&ctl->s_full[gj & 1]), (gj >> 1) & 1, smem_u32(&ctl->o_done[gj & 1]),
+                          ((gj - 2) >> 1) & 1);
+        } else {
+          mbar_wait(smem_u32(&ctl->s_full[gj & 1]), (gj >> 1) & 1);
+        }
+        tc_fence_after();
+        uint32_t s[32];
+        tmem_ld16x256_x8(tS + (gj & 1) * BN, s);
+        tmem_ld_wait();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&ctl->s_free[gj & 1]));   // QK(gj+2) may overwrite S(gj)
+
+        float xa[16], xb[16];
+#pragma unroll
+        for (int g = 0; g < 8; ++g) {
+          xa[2 * g] = __uint_as_float(s[4 * g]);
+          xa[2 * g + 1] = __uint_as_float(s[4 * g + 1]);
+          xb[2 * g] = __uint_as_float(s[4 * g + 2]);
+          xb[2 * g + 1] = __uint_as_float(s[4 * g + 3]);
+        }
+        if (k0 + BN - 1 > q0) {
+          const int qrA = q0 + rA, qrB = qrA + 8;
+#pragma unroll
+          for (int g = 0; g < 8; ++g) {
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+              const int key = k0 + 8 * g + 2 * quad + e;
+              xa[2 * g + e] = (key <= qrA) ? xa[2 * g + e] : -INFINITY;
+              xb[2 * g + e] = (key <= qrB) ? xb[2 * g + e] : -INFINITY;
+            }
+          }
+        }
+        float mxA = fmaxf(xa[0], xa[1]), mxB = fmaxf(xb[0], xb[1]);
+#pragma unroll
+        for (int c = 2; c < 16; c += 2) {
+          mxA = fmax3(mxA, xa[c], xa[c + 1]);
+          mxB = fmax3(mxB, xb[c], xb[c + 1]);
+        }
+        const bool any = __any_sync(0xffffffffu, (fmaf(mxA, sc, -mA) > 8.0f) || (fmaf(mxB, sc, -mB) > 8.0f));
+        float mA_new = mA, mB_new = mB, alphaA = 1.0f, alphaB = 1.0f;
+        if (any) {
+          mxA = fmaxf(mxA, __shfl_xor_sync(0xffffffffu, mxA, 1));
+          mxB = fmaxf(mxB, __shfl_xor_sync(0xffffffffu, mxB, 1));
+          mxA = fmaxf(mxA, __shfl_xor_sync(0xffffffffu, mxA, 2));
+          mxB = fmaxf(mxB, __shfl_xor_sync(0xffffffffu, mxB, 2));
+          mA_new = fmaxf(mA, mxA * sc);
+          mB_new = fmaxf(mB, mxB * sc);
+          alphaA = ex2_approx(mA - mA_new);
+          alphaB = ex2_approx(mB - mB_new);
+        }
+        float2 sumA2 = make_float2(0.f, 0.f), sumB2 = make_float2(0.f, 0.f);
+        const float2 sc2 = make_float2(sc, sc);
+        const float2 nmA = make_float2(-mA_new, -mA_new), nmB = make_float2(-mB_new, -mB_new);
+        uint32_t pr[16];
+#pragma unroll
+        for (int g = 0; g < 8; ++g) {
+          const float2 ta = ffma2(make_float2(xa[2 * g], xa[2 * g + 1]), sc2, nmA);
+          const float2 tb = ffma2(make_float2(xb[2 * g], xb[2 * g + 1]), sc2, nmB);
+          const float2 ea = make_float2(ex2_approx(ta.x), ex2_approx(ta.y));
+          const float2 eb = make_float2(ex2_approx(tb.x), ex2_approx(tb.y));
+          sumA2 = fadd2(sumA2, ea);
+          sumB2 = fadd2(sumB2, eb);
+          pr[2 * g] = pack_bf16x2(ea.x, ea.y);
+          pr[2 * g + 1] = pack_bf16x2(eb.x, eb.y);
+        }
+        lA = lA * alphaA + (sumA2.x + sumA2.y);
+        lB = lB * alphaB + (sumB2.x + sumB2.y);
+        mA = mA_new;
+        mB = mB_new;
+
+        if (any && j > 0) {
+          // the rare rescale touches O: every earlier PV of this item must be done (they complete in order)
+          mbar_wait(smem_u32(&ctl->o_done[(gj - 1) & 1]), ((gj - 1) >> 1) & 1);
+          tc_fence_after();
+#pragma unroll
+          for (int c0 = 0; c0 < D; c0 += 64) {
+            uint32_t o[32];
+            tmem_ld16x256_x8(tO + c0, o);
+            tmem_ld_wait();
+#pragma unroll
+            for (int g = 0; g < 8; ++g) {
+              o[4 * g] = __float_as_uint(__uint_as_float(o[4 * g]) * alphaA);
+              o[4 * g + 1] = __float_as_uint(__uint_as_float(o[4 * g + 1]) * alphaA);
+              o[4 * g + 2] = __float_as_uint(__uint_as_float(o[4 * g + 2]) * alphaB);
+              o[4 * g + 3] = __float_as_uint(__uint_as_float(o[4 * g + 3]) * alphaB);
+            }
+            tmem_st16x256_x8(tO + c0, o);
+          }
+          tmem_st_wait();
+        }
+        tmem_st16x128_x8(tP + (gj & 1) * C::kPStride, pr);
+        tmem_st_wait();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&ctl->p_full[gj & 1]));
+        if constexpr (PIECE) tmem_st16x128_x4(tQnext + 16 * pc, qn);   // completes under the next iteration
+        ++gj;
+      };
+
+      const int n_main = n_it >= kQChunks ? n_it - kQChunks : n_it;
+      int j = 0;
+      for (; j < n_main; ++j) {
+        if (j == 1) TR(0, n, 1);
+        iteration(j, std::false_type{}, nullptr, 0);
+      }
+      bool pieces = false;
+      if (j < n_it) {
+        // the last kQChunks iterations: is the next item posted and not empty?
+        const int nb = (n + 1) & 1;
+        bool have = mbar_try_wait(smem_u32(&ctl->list_full[nb]), ((n + 1) >> 1) & 1);
+        have = __all_sync(0xffffffffu, have);
+        pieces = have && ctl->item[nb] >= 0 && ctl->n_valid[nb] > 0;
+        if (pieces) {
+          const ItemP nx = read_item(ctl, nb);
+          const uint16_t* qnA =
+              p.Q + nx.b * p.qsb + nx.h * p.qsh + static_cast<int64_t>(nx.q0 + rA) * p.qsn + 2 * quad;
+          for (int pc = 0; j < n_it; ++j, ++pc) iteration(j, std::true_type{}, qnA, pc);
+        } else {
+          for (; j < n_it; ++j) iteration(j, std::false_type{}, nullptr, 0);
+        }
+      }
+      // ---- item boundary -----------------------------------------------------------------------------------------
+      TR(0, n, 2);
+      if (pieces) {
+        post_q();           // the pieces are in TMEM: QK(0) of the next item may start now
+        q_ready = true;
+      } else {
+        // not fetched during the loop (short item, or the scheduler was late): fetch it now, while the last PV
+        // drains.  The other Q buffer is free: its item's QKs completed before this item's first s_full.
+        const int nb = (n + 1) & 1;
+        mbar_wait(smem_u32(&ctl->list_full[nb]), ((n + 1) >> 1) & 1);
+        if (ctl->item[nb] >= 0 && ctl->n_valid[nb] > 0) {
+          put_q(read_item(ctl, nb), tQnext);
+          q_ready = true;
+        }
+      }
+      // ---- epilogue: O / l -> bf16 -> global -----------------------------------------------------------------
+      TR(0, n, 3);
+      mbar_wait(smem_u32(&ctl->o_done[(gj - 1) & 1]), ((gj - 1) >> 1) & 1);
+      tc_fence_after();
+      TR(0, n, 4);
+      lA += __shfl_xor_sync(0xffffffffu, lA, 1);
+      lB += __shfl_xor_sync(0xffffffffu, lB, 1);
+      lA += __shfl_xor_sync(0xffffffffu, lA, 2);
+      lB += __shfl_xor_sync(0xffffffffu, lB, 2);
+      const float invA = 1.0f / lA, invB = 1.0f / lB;
+#ifdef BSA_TRACE
+      if (trace_on && n < 32) g_tr[1][n][0] = clock64();
+#endif
+      const ItemP it = read_item(ctl, buf);
+      uint16_t* orowA = p.O + it.b * p.qsb + it.h * p.qsh + static_cast<int64_t>(q0 + rA) * p.qsn;
+      uint16_t* orowB = orowA + 8 * p.qsn;
+      // All of O into registers first, then the two arrivals, then the stores: mbarrier.arrive has release
+      // semantics, and an arrival AFTER the global stores waited ~800 clk for them (clock64 trace).
+      uint32_t o[D / 64][32];
+#pragma unroll
+      for (int c = 0; c < D / 64; ++c) tmem_ld16x256_x8(tO + 64 * c, o[c]);
+      tmem_ld_wait();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) {
+        mbar_arrive(smem_u32(&ctl->o_free));          // the next item's first PV may overwrite O
+        mbar_arrive(smem_u32(&ctl->list_free[buf]));  // nothing of this item's list / ctl fields is read below
+      }
+#ifdef BSA_TRACE
+      if (trace_on && n < 32) g_tr[1][n][2] = clock64();
+#endif
+#pragma unroll
+      for (int c = 0; c < D / 64; ++c) {
+        uint32_t wa[8], wb[8];
+#pragma unroll
+        for (int g = 0; g < 8; ++g) {
+          wa[g] = pack_bf16x2(__uint_as_float(o[c][4 * g]) * invA, __uint_as_float(o[c][4 * g + 1]) * invA);
+          wb[g] = pack_bf16x2(__uint_as_float(o[c][4 * g + 2]) * invB, __uint_as_float(o[c][4 * g + 3]) * invB);
+        }
+#pragma unroll
+        for (int g0 = 0; g0 < 8; g0 += 4) {
+          const uint4 va = quad_gather(wa[g0], wa[g0 + 1], wa[g0 + 2], wa[g0 + 3], quad);
+          const uint4 vb = quad_gather(wb[g0], wb[g0 + 1], wb[g0 + 2], wb[g0 + 3], quad);
+          *reinterpret_cast<uint4*>(orowA + 64 * c + 8 * (g0 + quad)) = va;
+          *reinterpret_cast<uint4*>(orowB + 64 * c + 8 * (g0 + quad)) = vb;
+        }
+      }
+#ifdef BSA_TRACE
+      if (trace_on && n < 32) g_tr[1][n][5] = clock64();
+#endif
+      if (p.lse && quad == 0) {
+        float* lse = p.lse + (static_cast<int64_t>(it.b) * p.H + it.h) * p.N + q0 + rA;
+        lse[0] = (mA + log2f(lA)) * 0.6931471805599453f;
+        lse[8] = (mB + log2f(lB)) * 0.6931471805599453f;
+      }
+#ifdef BSA_TRACE
+      TR(0, n, 5);
+      if (trace_on && n < 32) g_tr[0][n][6] = n_it;
+#endif
+    }
+  }
+
+  // ---- teardown ------------------------------------------------------------------------------------
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 4) tmem_dealloc<C::TMEM_COLS>(tmem);
+  if (tid == 0) {
+    // the last CTA of the launch returns the work counter to zero for the launch that takes this slot next
+    __threadfence();
+    if (atomicAdd(&g_work_done[cslot], 1u) == gridDim.x - 1) {
+      g_work_counter[cslot] = 0u;
+      g_work_done[cslot] = 0u;
+      __threadfence();
+    }
+  }
+}
+
 // ---- host side ---------------------------------------------------------------------------------
 template <int BM, int D, bool SPARSE>
 bsa_status run(const Dims& S, const void* Q, const void* K, const void* V, const Params& prm,
@@ -859,11 +1427,48 @@ bsa_status run(const Dims& S, const void* Q, const void* K, const void* V, const
   return check_launch("attn_kernel");
 }
 
+
+template <int D>
+bsa_status run_persistent(const Dims& S, const void* K, const void* V, const Params& prm, cudaStream_t stream) {
+  using C = Cfg<64, D>;
+  static std::atomic<unsigned> ticket{0};
+  CUtensorMap tk, tv;
+  if (!make_tmap_bhnd(&tk, K, S.B, S.Hkv, S.N, S.d, S.ksb, S.ksh, S.ksn, BN, S.d / 64, 1) ||
+      !make_tmap_bhnd(&tv, V, S.B, S.Hkv, S.N, S.d, S.ksb, S.ksh, S.ksn, BN, S.d / 64, 1))
+    return fail(BSA_ERR_CUDA, "attn: cuTensorMapEncodeTiled failed");
+  auto kern = attn64p_kernel<D>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM);
+  if (e != cudaSuccess) return fail(BSA_ERR_CUDA, "attn: smem attribute: %s", cudaGetErrorString(e));
+  const long long items = static_cast<long long>(prm.NT) * prm.B * prm.H;
+  const long long slots = static_cast<long long>(sm_count()) * C::kOcc;
+  const unsigned grid = static_cast<unsigned>(items < slots ? items : slots);
+  const int cslot = static_cast<int>(ticket.fetch_add(1u) % kCounterSlots);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(kThreadsP);
+  cfg.dynamicSmemBytes = C::SMEM;
+  cfg.stream = stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = prm.pdl ? 1 : 0;
+  e = cudaLaunchKernelEx(&cfg, kern, tk, tv, prm, static_cast<int>(items), cslot);
+  if (e != cudaSuccess) return fail(BSA_ERR_CUDA, "attn: cudaLaunchKernelEx: %s", cudaGetErrorString(e));
+  return check_launch("attn64p_kernel");
+}
+
 }  // namespace
 
 // The transposed kernel of attn_t.cu (keys on the M dimension, M = 128) is parity-green but slower than
 // the M = 64 kernel here on B200 (C2: 2.3-2.7 ms against 1.5 ms; ablation in DESIGN.md section 6), so it
 // is an opt-in experiment: the environment variable BSA_ATTN_T=1 routes block 64 / head_dim 128 to it.
+// BSA_ATTN_PERSISTENT=0 routes block 64 back to the one-CTA-per-item kernel (A/B runs).
+static bool attn_persistent_enabled() {
+  const char* e = getenv("BSA_ATTN_PERSISTENT");
+  return e == nullptr || e[0] != '0';
+}
+
 static bool attn_t_enabled() {
   const char* e = getenv("BSA_ATTN_T");
   return e != nullptr && e[0] == '1';
@@ -893,6 +1498,12 @@ bsa_status launch_attn(const Dims& S, const void* Q, const void* K, const void* 
   if (sparse) {
     if (!bitmap && W > kMaxW) return fail(BSA_ERR_UNSUPPORTED, "sparse attn: kv_width %d > %d", W, kMaxW);
     prm.NT = S.NB;
+    if (S.Bn == 64 && !bitmap && W <= kMaxWP && attn_persistent_enabled() &&
+        static_cast<long long>(S.NB) * S.B * S.H < (1ll << 31)) {
+      if (S.d == 64) return run_persistent<64>(S, K, V, prm, stream);
+      if (S.d == 128) return run_persistent<128>(S, K, V, prm, stream);
+      if (S.d == 256) return run_persistent<256>(S, K, V, prm, stream);
+    }
 #define BSA_SP(BMM, DD) \
   if (S.Bn == BMM && S.d == DD) return run<BMM, DD, true>(S, Q, K, V, prm, stream);
     BSA_SP(64, 64) BSA_SP(64, 128) BSA_SP(64, 256) BSA_SP(128, 64) BSA_SP(128, 128) BSA_SP(128, 256)
