@@ -521,7 +521,10 @@ def run_gpu(args):
         "wall_ms_timed_region": wall_ms,
         "kv_count_sum": kv_sum,
         "mean_blocks_per_tile": head["mean_blocks_per_tile"],
-        "roofline": {"bound": "tensor", "kernel": "attn_kernel<sparse> (bsa_sparse_attn_fwd)",
+        "roofline": {"bound": "tensor",
+                     "kernel": ("attn64p_kernel (bsa_sparse_attn_fwd; persistent, 64-token blocks)"
+                                if cfg.block == 64 and cfg.k_budget * 2 <= 128 else
+                                "attn_kernel<sparse> (bsa_sparse_attn_fwd)"),
                      "achieved": tf_sparse, "peak": peak_tf, "unit": "TFLOP/s", "frac": tf_sparse / peak_tf,
                      "traffic": ncu_traffic(f"attn_sparse/{args.workload}/{args.policy}"),
                      "peak_source": f"{peaks['_source']} bf16_tflops_sustained",

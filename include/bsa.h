@@ -13,7 +13,10 @@
  * Conventions
  *   - Every pointer named Q/K/V/O/meta/kv_idx/kv_count/sigma/sigma_bar/trigger/tau/lse/workspace is a
  *     DEVICE pointer owned by the caller; the library allocates no device memory and keeps no state
- *     between calls (bsa_select_static is the one exception: a static device array, see there).
+ *     between calls.  Two exceptions, both small static device arrays: the scratch of bsa_select_static (see
+ *     there) and the work counters of the persistent sparse attention kernel -- a launch takes one of 1024
+ *     counter slots and returns it to zero itself; launches that overlap on the GPU use different slots unless
+ *     more than 1024 of them are in flight at once.
  *     `shape` is a HOST pointer.  `stream` is a cudaStream_t passed as void*.
  *   - Every call only enqueues work on `stream`; it never synchronises and never touches the
  *     default stream.

@@ -1004,3 +1004,106 @@ def test_select_attn_one_call(bsa, name, policy):
     ref, _ = oracle.attn_pairs(inp.Q, inp.K, inp.V, cfg.block, pairs, orc["kv_idx"], orc["kv_count"])
     Og = O1[0].float().cpu().numpy().reshape(H, T, cfg.block, cfg.head_dim)
     compare_attn(np.stack([Og[h, t] for t, h in pairs]), ref, f"one-call {name}/{policy}")
+
+
+# ---- the persistent block-64 attention kernel against the one-CTA-per-item kernel ----------------------------
+def _attn_both_kernels(bsa, Q, K, V, kv_idx, kv_count, block):
+    """(O, lse) of the persistent kernel and of the per-item kernel (BSA_ATTN_PERSISTENT=0) on the same lists"""
+    import torch
+    out = []
+    for flag in ("1", "0"):
+        os.environ["BSA_ATTN_PERSISTENT"] = flag
+        try:
+            O, lse = bsa.bsa_sparse_attn_fwd(Q, K, V, kv_idx, kv_count, block, want_lse=True)
+            torch.cuda.synchronize()
+        finally:
+            os.environ.pop("BSA_ATTN_PERSISTENT", None)
+        out.append((O, lse))
+    return out
+
+
+@pytest.mark.parametrize("d", [64, 128, 256])
+def test_persistent_attention_item_boundaries(bsa, d):
+    """Hand-made kv_idx rows that stress what is new in the persistent kernel -- items of 0, 1, 2, 3 and many
+    blocks in every order (runs of empty items, the first and the last item of a CTA empty, lists shorter than
+    the number of Q-tile pieces, duplicates, sentinels, future blocks) -- give bit-identical O and lse in both
+    kernels, and the result matches the oracle."""
+    import dataclasses
+    import torch
+    key = f"persist{d}"
+    if key not in _CACHE:
+        cfg = dataclasses.replace(synth.CONFIGS["C1"], name=key, number=80 + d // 64, seqlen=40 * 64, n_q_heads=6,
+                                  n_kv_heads=2, head_dim=d, block=64)
+        _CACHE[key] = (cfg, synth.make_inputs(cfg), None)
+    cfg, inp, _ = _CACHE[key]
+    Q, K, V = _dev(inp)
+    T, H, NB, W = cfg.n_blocks, cfg.n_q_heads, cfg.n_blocks, 24
+    rng = np.random.default_rng(1234 + d)
+    idx = np.full((H, T, W), NB, dtype=np.int32)
+    cnt = np.zeros((H, T), dtype=np.int32)
+    lengths = [0, 0, 1, 2, 3, 0, 4, 5, 9, 17, 24, 0, 0, 0, 7, 1, 0, 12]
+    for h in range(H):
+        for t in range(T):
+            n = lengths[(h * 7 + t * 3 + (t // 5)) % len(lengths)]
+            n = min(n, t + 1)
+            row = rng.permutation(t + 1)[:n].astype(np.int32)
+            fill = list(row)
+            if n >= 3:
+                fill.insert(1, row[0])              # a duplicate
+                fill.insert(2, NB)                  # a sentinel inside the counted part
+            if t + 1 < NB and n >= 2:
+                fill.insert(0, t + 1)               # a block from the future
+            fill = fill[:W]
+            idx[h, t, :len(fill)] = fill
+            cnt[h, t] = len(fill)
+    idx[:, T - 1, :] = NB                           # the heaviest-first order starts with empty items
+    cnt[:, T - 1] = W
+    idx[:, 0, :] = NB                               # ... and ends with them
+    kv_idx = torch.from_numpy(idx)[None].cuda()
+    kv_count = torch.from_numpy(cnt)[None].cuda()
+    (Op, lp), (Oi, li) = _attn_both_kernels(bsa, Q, K, V, kv_idx, kv_count, 64)
+    assert torch.equal(Op.view(torch.int16), Oi.view(torch.int16))
+    assert torch.equal(lp.view(torch.int32), li.view(torch.int32))
+    pairs = [(t, h) for h in range(H) for t in range(T)]
+    ref, ref_lse = oracle.attn_pairs(inp.Q, inp.K, inp.V, 64, pairs, idx, cnt)
+    got = Op[0].float().cpu().numpy().reshape(H, T, 64, d)
+    compare_attn(np.stack([got[h, t] for t, h in pairs]), ref, f"persistent d={d}")
+    glse = lp[0].cpu().numpy().reshape(H, T, 64)
+    fin = np.isfinite(ref_lse)
+    assert np.array_equal(np.isneginf(np.stack([glse[h, t] for t, h in pairs])), ~fin)
+    np.testing.assert_allclose(np.stack([glse[h, t] for t, h in pairs])[fin], ref_lse[fin], rtol=0, atol=LSE_TOL)
+
+
+def test_persistent_attention_full_size_and_streams(bsa):
+    """C2 router_quest: the persistent kernel's O equals the per-item kernel's bit for bit; two launches that
+    overlap on different streams (each takes its own work counter) give the results of running them alone;
+    rows wider than the persistent kernel's 128 entries take the per-item kernel."""
+    import torch
+    cfg, inp, _ = _case("C2")
+    Q, K, V = _dev(inp)
+    buf = bsa.bsa_build_block_meta(K, cfg.block, 3)
+    r = bsa.bsa_select(Q, buf, K, cfg.block, "router_quest", cfg.k_budget, 0.25)
+    r2 = bsa.bsa_select(Q, buf, K, cfg.block, "topk", cfg.k_budget, 0.25)
+    (Op, lp), (Oi, li) = _attn_both_kernels(bsa, Q, K, V, r["kv_idx"], r["kv_count"], cfg.block)
+    assert torch.equal(Op.view(torch.int16), Oi.view(torch.int16)) and torch.equal(lp, li)
+    O2, _ = bsa.bsa_sparse_attn_fwd(Q, K, V, r2["kv_idx"], r2["kv_count"], cfg.block)
+    torch.cuda.synchronize()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    Oa, Ob = torch.empty_like(Q), torch.empty_like(Q)
+    for rep in range(4):
+        with torch.cuda.stream(s1):
+            bsa.bsa_sparse_attn_fwd(Q, K, V, r["kv_idx"], r["kv_count"], cfg.block, O=Oa)
+        with torch.cuda.stream(s2):
+            bsa.bsa_sparse_attn_fwd(Q, K, V, r2["kv_idx"], r2["kv_count"], cfg.block, O=Ob)
+        torch.cuda.synchronize()
+        assert torch.equal(Oa.view(torch.int16), Op.view(torch.int16)), rep
+        assert torch.equal(Ob.view(torch.int16), O2.view(torch.int16)), rep
+        Oa.zero_()
+        Ob.zero_()
+    # W = 160 > 128: same lists padded with sentinels
+    pad = torch.full((*r["kv_idx"].shape[:3], 160 - r["kv_idx"].shape[3]), cfg.n_blocks, dtype=torch.int32,
+                     device="cuda")
+    wide = torch.cat([r["kv_idx"], pad], dim=3).contiguous()
+    Ow, _ = bsa.bsa_sparse_attn_fwd(Q, K, V, wide, r["kv_count"], cfg.block)
+    torch.cuda.synchronize()
+    assert torch.equal(Ow.view(torch.int16), Op.view(torch.int16))
