@@ -3,17 +3,25 @@
 // kv_idx with a single-compare sentinel skip), and the dense causal kernel of the same design
 // (L45, L156) used as the "x dense" denominator.
 //
-// One CTA per (Q tile, head, batch); 7 warps:
+// Two kernels:
+//   attn64p_kernel<D>        sparse attention at 64-token blocks from kv_idx rows of up to 128 entries -- the
+//                            paper's configuration.  Persistent: 2 x #SM CTAs walk the (tile, head) items; Q, S,
+//                            P and O all live in TMEM (two half-lane planes), only K / V pass through shared
+//                            memory.  Described at its definition below.
+//   attn_kernel<BM,D,SPARSE> one CTA per (Q tile, head, batch): dense attention (BM = 128), sparse attention at
+//                            128-token blocks, bitmap lists, rows wider than 128 entries, and the A/B reference
+//                            of the persistent kernel (BSA_ATTN_PERSISTENT=0).  7 warps:
 //   warps 0-3  softmax: tcgen05.ld of S, fp32 online softmax in base 2, P (bf16) -> shared memory
-//              (BM = 128) or back into TMEM over the S buffer just read (BM = 64: PV then takes its A
-//              operand from TMEM), lazy rescale of the O accumulator in TMEM, final normalisation and store
-//   warp 4     TMA producer: Q once, then K and V 64-key sub-blocks through a ring of stages; the
-//              row coordinate of each load is kv_idx * block ("gather" = ordinary tiled TMA loads)
-//   warp 5     one thread issues tcgen05.mma: S = Q K^T (both K-major, 128B swizzle) into TMEM and,
-//              for BM = 128 with d <= 128, O += P V (V is the MN-major B operand) into TMEM
+//              (BM = 128) or into TMEM (BM = 64: PV then takes its A operand from TMEM), lazy rescale of the
+//              O accumulator in TMEM, final normalisation and store
+//   warp 4     TMA producer: Q once (BM = 128; for BM = 64 the softmax warps put Q into TMEM), then K and V
+//              64-key sub-blocks through a ring of stages; the row coordinate of each load is
+//              kv_idx * block ("gather" = ordinary tiled TMA loads)
+//   warp 5     one thread issues tcgen05.mma: S = Q K^T into TMEM (SS form, both K-major, 128B swizzle; BM = 64:
+//              TS form, A = Q from TMEM) and, for BM = 128 with d <= 128, O += P V (V is the MN-major B operand)
 //   warp 6     BM = 64 and d = 256: a second thread issues the O += P V MMAs (own V ring, see below)
 // Q tile rows: sparse = one selection tile (BM = block), dense = 128.  For BM = 64 the accumulator
-// rows live in lanes 0-15 of each TMEM sub-partition (UMMA M = 64 layout).
+// rows live in lanes 0-15 (or, with a lane offset of 16 in the address, 16-31) of each TMEM sub-partition.
 #include <cuda_bf16.h>
 #include <stdlib.h>
 

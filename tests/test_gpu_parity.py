@@ -1090,16 +1090,18 @@ def test_persistent_attention_full_size_and_streams(bsa):
     torch.cuda.synchronize()
     s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
     Oa, Ob = torch.empty_like(Q), torch.empty_like(Q)
-    for rep in range(4):
+    for rep in range(12):
+        # (torch's side streams do not synchronise with the default stream: the outputs are cleared on the
+        # stream that writes them next)
         with torch.cuda.stream(s1):
+            Oa.zero_()
             bsa.bsa_sparse_attn_fwd(Q, K, V, r["kv_idx"], r["kv_count"], cfg.block, O=Oa)
         with torch.cuda.stream(s2):
+            Ob.zero_()
             bsa.bsa_sparse_attn_fwd(Q, K, V, r2["kv_idx"], r2["kv_count"], cfg.block, O=Ob)
         torch.cuda.synchronize()
         assert torch.equal(Oa.view(torch.int16), Op.view(torch.int16)), rep
         assert torch.equal(Ob.view(torch.int16), O2.view(torch.int16)), rep
-        Oa.zero_()
-        Ob.zero_()
     # W = 160 > 128: same lists padded with sentinels
     pad = torch.full((*r["kv_idx"].shape[:3], 160 - r["kv_idx"].shape[3]), cfg.n_blocks, dtype=torch.int32,
                      device="cuda")
