@@ -1436,10 +1436,12 @@ bsa_status run(const Dims& S, const void* Q, const void* K, const void* V, const
 }
 
 
+// one ticket sequence for every head_dim instantiation: two launches in flight never share a counter slot
+std::atomic<unsigned> g_ticket{0};
+
 template <int D>
 bsa_status run_persistent(const Dims& S, const void* K, const void* V, const Params& prm, cudaStream_t stream) {
   using C = Cfg<64, D>;
-  static std::atomic<unsigned> ticket{0};
   CUtensorMap tk, tv;
   if (!make_tmap_bhnd(&tk, K, S.B, S.Hkv, S.N, S.d, S.ksb, S.ksh, S.ksn, BN, S.d / 64, 1) ||
       !make_tmap_bhnd(&tv, V, S.B, S.Hkv, S.N, S.d, S.ksb, S.ksh, S.ksn, BN, S.d / 64, 1))
@@ -1450,7 +1452,7 @@ bsa_status run_persistent(const Dims& S, const void* K, const void* V, const Par
   const long long items = static_cast<long long>(prm.NT) * prm.B * prm.H;
   const long long slots = static_cast<long long>(sm_count()) * C::kOcc;
   const unsigned grid = static_cast<unsigned>(items < slots ? items : slots);
-  const int cslot = static_cast<int>(ticket.fetch_add(1u) % kCounterSlots);
+  const int cslot = static_cast<int>(g_ticket.fetch_add(1u) % kCounterSlots);
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(grid);
   cfg.blockDim = dim3(kThreadsP);

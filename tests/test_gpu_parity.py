@@ -1088,8 +1088,14 @@ def test_persistent_attention_full_size_and_streams(bsa):
     assert torch.equal(Op.view(torch.int16), Oi.view(torch.int16)) and torch.equal(lp, li)
     O2, _ = bsa.bsa_sparse_attn_fwd(Q, K, V, r2["kv_idx"], r2["kv_count"], cfg.block)
     torch.cuda.synchronize()
-    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
-    Oa, Ob = torch.empty_like(Q), torch.empty_like(Q)
+    # a third, concurrent launch of another head_dim instantiation (d = 64): its own counter slot too
+    cfg1, inp1, _ = _case("C1")
+    Q1, K1, V1 = _dev(inp1)
+    r1 = bsa.bsa_select(Q1, bsa.bsa_build_block_meta(K1, cfg1.block, 3), K1, cfg1.block, "router", cfg1.k_budget, 0.25)
+    O1, _ = bsa.bsa_sparse_attn_fwd(Q1, K1, V1, r1["kv_idx"], r1["kv_count"], cfg1.block)
+    torch.cuda.synchronize()
+    s1, s2, s3 = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
+    Oa, Ob, Oc = torch.empty_like(Q), torch.empty_like(Q), torch.empty_like(Q1)
     for rep in range(12):
         # (torch's side streams do not synchronise with the default stream: the outputs are cleared on the
         # stream that writes them next)
@@ -1099,9 +1105,14 @@ def test_persistent_attention_full_size_and_streams(bsa):
         with torch.cuda.stream(s2):
             Ob.zero_()
             bsa.bsa_sparse_attn_fwd(Q, K, V, r2["kv_idx"], r2["kv_count"], cfg.block, O=Ob)
+        with torch.cuda.stream(s3):
+            Oc.zero_()
+            for _ in range(3):
+                bsa.bsa_sparse_attn_fwd(Q1, K1, V1, r1["kv_idx"], r1["kv_count"], cfg1.block, O=Oc)
         torch.cuda.synchronize()
         assert torch.equal(Oa.view(torch.int16), Op.view(torch.int16)), rep
         assert torch.equal(Ob.view(torch.int16), O2.view(torch.int16)), rep
+        assert torch.equal(Oc.view(torch.int16), O1.view(torch.int16)), rep
     # W = 160 > 128: same lists padded with sentinels
     pad = torch.full((*r["kv_idx"].shape[:3], 160 - r["kv_idx"].shape[3]), cfg.n_blocks, dtype=torch.int32,
                      device="cuda")
